@@ -1,0 +1,148 @@
+/*
+ * rad.h -- C ABI of the B200 (sm_100a) FP64 radiation-integral evaluator.
+ *
+ * The operation (arXiv 1910.10391, cited by line of PAPER.md):
+ *
+ *   d2I/(dw dOmega) = e^2/4pi^2 | int f(t,n) e^{i w (t - n.x(t))} dt |^2        eq. (1)
+ *
+ * in the paper's small-angle, leading-order expanded form -- f_x, f_y, f_z of
+ * eqs. (3)-(5), g of eq. (6), phase of eq. (7)
+ * -- evaluated for EVERY point of a tensor grid (w, n_x, n_y) over
+ * one sampled trajectory ("the integral over the same trajectory N_x x N_y x N_w
+ * times"; result "saved in a cube"), classically or
+ * with the semi-classical substitution w -> w* = w/(1 - hbar w/E):
+ *
+ *   spin-0   (substitution model) out = (w/w*) classical(w*)                     eq. (9),
+ *   spin-1/2 (BCK model)          out = [ (E*^2+E^2)/2E^2 |I|^2
+ *                                       + w^2/(2 E^2 gamma^2) |J|^2 ] / 4pi^2    eqs. (10)-(12)
+ *
+ * and summed over trajectories / crystal sections.
+ * The time integral is the composite trapezoid rule on the given samples
+ * (reading Q1); the acceleration is zero outside [t_0, t_{n-1}] (Q2).
+ *
+ * Units: c = 1; t, x, y, dz in one length unit (metres in all shipped workloads);
+ * v dimensionless; accelerations per length; omega in rad per length.  Output in
+ * units of e^2 (multiply by alpha = 1/137.036 for hbar = c = 1), 1/4pi^2 included.
+ *
+ * Conventions common to all calls
+ *   - Every `const double*` inside rad_traj / rad_traj_batch / rad_grid and every
+ *     `out` is DEVICE memory owned by the caller, 8-byte aligned, read-only for the
+ *     inputs.  The *_host entry points at the end take HOST memory instead.
+ *   - `workspace` is caller-owned DEVICE scratch of at least rad_workspace_bytes()
+ *     bytes, 256-byte aligned.  If NULL, scratch is taken from the device's
+ *     stream-ordered pool (cudaMallocAsync / cudaFreeAsync on `cuda_stream`) and
+ *     released in stream order.  The library keeps no pointer past the enqueued work
+ *     and allocates nothing persistent.
+ *   - `cuda_stream` is a cudaStream_t (NULL = legacy default stream).  All work is
+ *     enqueued on it; no call synchronises the host (the *_host calls do, once, at
+ *     the end).
+ *   - Cube order: out[(i_w * n_thy + i_y) * n_thx + i_x]  (theta_x fastest).
+ *   - Return value: RAD_OK (0) or a negative rad_status; nothing throws or aborts.
+ *     Not checked (garbage in, NaN/inf out): non-monotone t, q <= 0, non-finite
+ *     samples.  A grid point with u = omega * hbarc_over_E >= 1 (photon energy above
+ *     the particle energy, no final state) yields NaN at that point (the omega array
+ *     lives on the device; no host-side check, no sync).
+ *   - Results are deterministic run to run (fixed reduction order, no FP atomics).
+ *   - There is no CPU fallback: without a CUDA device every compute call returns
+ *     RAD_ECUDA.
+ */
+#ifndef RAD_H
+#define RAD_H
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef enum {
+    RAD_OK = 0,
+    RAD_EINVAL = -1,      /* null pointer, n < 2, empty grid, bad spin/model, misaligned pointer */
+    RAD_EDOMAIN = -2,     /* host-visible parameter outside the method's domain (hbarc_over_E < 0) */
+    RAD_ECUDA = -3,       /* CUDA runtime error; rad_strerror gives the CUDA text of the last one */
+    RAD_ENOSPACE = -4     /* workspace given but smaller than rad_workspace_bytes() */
+} rad_status;
+
+typedef enum { RAD_CLASSICAL = 0, RAD_SPIN0 = 1, RAD_SPIN_HALF = 2 } rad_model;
+
+/* One trajectory (or one crystal section), structure of arrays, n >= 2 samples.
+ * t: time; dz = z - beta0 t; x, y; vx, vy; dvz = v_z - beta0 (beta0 = 1 - 1/2gamma^2,
+ * PAPER.md:28); ax, ay, az: accelerations; gamma: Lorentz factor per sample (Q6:
+ * 1/2gamma_k^2 is used sample-wise, the J coefficient of eq. 10 uses gamma[0]). */
+typedef struct {
+    int64_t n;
+    const double *t, *dz, *x, *y, *vx, *vy, *dvz, *ax, *ay, *az, *gamma;
+} rad_traj;
+
+/* `count` trajectories; row p of each array starts at element p*stride and holds
+ * n[p] <= stride samples.  `n` is a HOST array (it sizes the launch). */
+typedef struct {
+    int32_t count;
+    int64_t stride;
+    const int64_t *n;
+    const double *t, *dz, *x, *y, *vx, *vy, *dvz, *ax, *ay, *az, *gamma;
+} rad_traj_batch;
+
+/* Tensor grid: omega[n_omega] >= 0 (rad/length), thx[n_thx] = n_x, thy[n_thy] = n_y
+ * (direction cosines, small; theta^2 = n_x^2 + n_y^2). */
+typedef struct {
+    int32_t n_omega, n_thx, n_thy;
+    const double *omega, *thx, *thy;
+} rad_grid;
+
+/* Classical spectrum, eq. (1) with eqs. (3)-(7).  out: n_omega*n_thy*n_thx doubles. */
+int rad_classical(const rad_traj *traj, const rad_grid *grid, double *out,
+                  void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* Semi-classical spectrum.  spin = 0: substitution model, eq. (9); spin = 1: spin-1/2,
+ * BCK eq. (10).  hbarc_over_E = hbar c / E in the length unit, so that
+ * u = hbar w / E = omega * hbarc_over_E and w* = omega / (1 - u). */
+int rad_semiclassical(const rad_traj *traj, const rad_grid *grid, int spin,
+                      double hbarc_over_E, double *out,
+                      void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* out[m] (+)= sum over p (ascending) of the spectrum of trajectory p.
+ * hbarc_over_E: HOST array, one per trajectory (NULL allowed iff model is classical).
+ * accumulate: 0 overwrites out, 1 adds to it (resume a partial ensemble). */
+int rad_ensemble_sum(const rad_traj_batch *batch, const rad_grid *grid, rad_model model,
+                     const double *hbarc_over_E, int accumulate, double *out,
+                     void *workspace, size_t workspace_bytes, void *cuda_stream);
+
+/* dI/dw[i_w] = sum_{i_x,i_y} cube * d_omega_solid, optionally only where
+ * n_x^2 + n_y^2 <= theta_cut^2 (theta_cut <= 0: no mask) -- the paper's "final sum over
+ * the spatial integrals", done on the device.  `cube` is the output of
+ * one of the calls above; spectrum: n_omega doubles (device). */
+int rad_angular_sum(const double *cube, const rad_grid *grid, double d_solid_angle,
+                    double theta_cut, double *spectrum, void *cuda_stream);
+
+/* Scratch needed by any call above for `count` trajectories of at most n_max samples on a
+ * grid of the given shape (count = 1 for the single-trajectory calls).  0 on bad input. */
+size_t rad_workspace_bytes(int32_t count, int64_t n_max,
+                           int32_t n_omega, int32_t n_thx, int32_t n_thy);
+
+/* HOST-buffer variants (the paper's flow: trajectory copied to the GPU once, cube copied
+ * back once).  Every pointer inside traj/batch/grid and `out` is HOST memory
+ * (pinned memory makes the copies asynchronous).  Device buffers come from the
+ * stream-ordered pool; the call returns after the result is in `out`.
+ * model: rad_model; hbarc_over_E ignored for RAD_CLASSICAL. */
+int rad_eval_host(const rad_traj *traj, const rad_grid *grid, rad_model model,
+                  double hbarc_over_E, double *out, void *cuda_stream);
+int rad_ensemble_sum_host(const rad_traj_batch *batch, const rad_grid *grid, rad_model model,
+                          const double *hbarc_over_E, int accumulate, double *out,
+                          void *cuda_stream);
+
+/* FP64 FMA peak of the current device, measured: runs a register-resident DFMA chain
+ * kernel for about `millis` ms and returns FLOP/s (2 per FMA lane); <= 0 on error. */
+double rad_measure_fp64_peak(double millis, void *cuda_stream);
+
+/* Number of kernels the library has launched in this process (bench bookkeeping). */
+int64_t rad_launch_count(void);
+
+/* Static text for a rad_status; for RAD_ECUDA the text of the last CUDA error seen. */
+const char *rad_strerror(int code);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* RAD_H */

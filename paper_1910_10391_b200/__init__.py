@@ -1,0 +1,25 @@
+"""B200 (sm_100a) FP64 radiation-integral evaluator -- thin Python binding.
+
+Argument marshalling only: every step of the hot path runs in the CUDA kernels of
+``csrc/rad.cu`` behind the C ABI of ``include/rad.h``.  PyTorch is used for device
+memory and streams.  There is no CPU fallback: if the shared library is missing or
+no CUDA device is visible, calls raise.
+
+Functions mirror the C entry points one to one:
+``rad_classical``, ``rad_semiclassical``, ``rad_ensemble_sum``, ``rad_angular_sum``,
+``rad_workspace_bytes``, ``rad_eval_host``, ``rad_ensemble_sum_host``,
+``rad_measure_fp64_peak``, ``rad_launch_count``.
+"""
+from __future__ import annotations
+
+from .binding import (CLASSICAL, FIELDS, SPIN0, SPIN_HALF, RadError, build_library, library_path,
+                      load_library, rad_angular_sum, rad_classical, rad_ensemble_sum,
+                      rad_ensemble_sum_host, rad_eval_host, rad_launch_count,
+                      rad_measure_fp64_peak, rad_semiclassical, rad_workspace_bytes)
+
+__all__ = [
+    "CLASSICAL", "SPIN0", "SPIN_HALF", "FIELDS", "RadError", "build_library", "library_path",
+    "load_library", "rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_angular_sum",
+    "rad_workspace_bytes", "rad_eval_host", "rad_ensemble_sum_host", "rad_measure_fp64_peak",
+    "rad_launch_count",
+]

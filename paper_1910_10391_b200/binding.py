@@ -1,0 +1,274 @@
+"""ctypes binding of ``include/rad.h`` (argument marshalling only; see package docstring)."""
+from __future__ import annotations
+
+import ctypes
+import os
+import subprocess
+from pathlib import Path
+
+import numpy as np
+import torch
+
+_PKG = Path(__file__).resolve().parent
+_SRC = _PKG / "csrc"
+_SO = _PKG / "librad_b200.so"
+
+CLASSICAL, SPIN0, SPIN_HALF = 0, 1, 2
+FIELDS = ("t", "dz", "x", "y", "vx", "vy", "dvz", "ax", "ay", "az", "gamma")
+
+EXPORTS = ("rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_angular_sum",
+           "rad_workspace_bytes", "rad_eval_host", "rad_ensemble_sum_host",
+           "rad_measure_fp64_peak", "rad_launch_count", "rad_strerror")
+
+_dp = ctypes.POINTER(ctypes.c_double)
+_lib = None
+
+
+class RadError(RuntimeError):
+    def __init__(self, code: int, text: str):
+        super().__init__(f"rad status {code}: {text}")
+        self.code = code
+
+
+class _Traj(ctypes.Structure):
+    _fields_ = [("n", ctypes.c_int64)] + [(k, ctypes.c_void_p) for k in FIELDS]
+
+
+class _Batch(ctypes.Structure):
+    _fields_ = ([("count", ctypes.c_int32), ("stride", ctypes.c_int64), ("n", ctypes.c_void_p)]
+                + [(k, ctypes.c_void_p) for k in FIELDS])
+
+
+class _Grid(ctypes.Structure):
+    _fields_ = [("n_omega", ctypes.c_int32), ("n_thx", ctypes.c_int32), ("n_thy", ctypes.c_int32),
+                ("omega", ctypes.c_void_p), ("thx", ctypes.c_void_p), ("thy", ctypes.c_void_p)]
+
+
+def library_path() -> Path:
+    return _SO
+
+
+def build_library(force: bool = False, verbose: bool = False) -> Path:
+    """Compile csrc/rad.cu for sm_100a into the in-tree shared library (nvcc cross-compiles
+    without a GPU)."""
+    srcs = [_SRC / "rad.cu", _SRC / "rad_device.cuh", _SRC / "sincos_coeffs.h",
+            _PKG.parent / "include" / "rad.h"]
+    if not force and _SO.exists() and all(_SO.stat().st_mtime >= s.stat().st_mtime for s in srcs):
+        return _SO
+    tmp = _SO.with_suffix(f".tmp{os.getpid()}.so")
+    cmd = ["nvcc", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
+           "-shared", "-Xcompiler", "-fPIC", "-o", str(tmp), str(srcs[0])]
+    if verbose:
+        cmd[1:1] = ["-Xptxas", "-v"]
+    subprocess.run(cmd, check=True)
+    os.replace(tmp, _SO)
+    return _SO
+
+
+def load_library() -> ctypes.CDLL:
+    """Load the C-ABI library.  Fails loudly if it has not been built."""
+    global _lib
+    if _lib is not None:
+        return _lib
+    if not _SO.exists():
+        raise FileNotFoundError(
+            f"{_SO} is missing: run __graft_entry__.build() (nvcc) first; there is no CPU fallback")
+    lib = ctypes.CDLL(str(_SO))
+    vp, sz, i32, i64, dbl = ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int32, ctypes.c_int64, ctypes.c_double
+    lib.rad_classical.argtypes = [ctypes.POINTER(_Traj), ctypes.POINTER(_Grid), vp, vp, sz, vp]
+    lib.rad_semiclassical.argtypes = [ctypes.POINTER(_Traj), ctypes.POINTER(_Grid), ctypes.c_int, dbl,
+                                      vp, vp, sz, vp]
+    lib.rad_ensemble_sum.argtypes = [ctypes.POINTER(_Batch), ctypes.POINTER(_Grid), ctypes.c_int, vp,
+                                     ctypes.c_int, vp, vp, sz, vp]
+    lib.rad_angular_sum.argtypes = [vp, ctypes.POINTER(_Grid), dbl, dbl, vp, vp]
+    lib.rad_workspace_bytes.argtypes = [i32, i64, i32, i32, i32]
+    lib.rad_workspace_bytes.restype = sz
+    lib.rad_eval_host.argtypes = [ctypes.POINTER(_Traj), ctypes.POINTER(_Grid), ctypes.c_int, dbl, vp, vp]
+    lib.rad_ensemble_sum_host.argtypes = [ctypes.POINTER(_Batch), ctypes.POINTER(_Grid), ctypes.c_int, vp,
+                                          ctypes.c_int, vp, vp]
+    lib.rad_measure_fp64_peak.argtypes = [dbl, vp]
+    lib.rad_measure_fp64_peak.restype = dbl
+    lib.rad_launch_count.restype = i64
+    lib.rad_strerror.argtypes = [ctypes.c_int]
+    lib.rad_strerror.restype = ctypes.c_char_p
+    for name in ("rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_angular_sum",
+                 "rad_eval_host", "rad_ensemble_sum_host"):
+        getattr(lib, name).restype = ctypes.c_int
+    _lib = lib
+    return lib
+
+
+def _check(rc: int) -> None:
+    if rc != 0:
+        raise RadError(rc, load_library().rad_strerror(rc).decode())
+
+
+def _dev(t: torch.Tensor, name: str) -> torch.Tensor:
+    if not isinstance(t, torch.Tensor) or not t.is_cuda or t.dtype != torch.float64 or not t.is_contiguous():
+        raise TypeError(f"{name}: expected a contiguous float64 CUDA tensor")
+    return t
+
+
+def _stream_ptr(stream) -> int:
+    if stream is None:
+        if not torch.cuda.is_available():
+            return 0           # the library itself then reports RAD_ECUDA: no CPU fallback
+        stream = torch.cuda.current_stream()
+    return int(stream.cuda_stream)
+
+
+def _grid_struct(omega, thx, thy) -> _Grid:
+    return _Grid(omega.numel(), thx.numel(), thy.numel(), omega.data_ptr(), thx.data_ptr(), thy.data_ptr())
+
+
+def _traj_struct(traj: dict) -> _Traj:
+    ts = [_dev(traj[k], k) for k in FIELDS]
+    n = ts[0].numel()
+    if any(t.ndim != 1 or t.numel() != n for t in ts):
+        raise ValueError("trajectory tensors must be 1-D and of one length")
+    return _Traj(n, *[t.data_ptr() for t in ts])
+
+
+def _ws_args(workspace):
+    if workspace is None:
+        return None, 0
+    if not workspace.is_cuda or not workspace.is_contiguous():
+        raise TypeError("workspace: expected a contiguous CUDA tensor")
+    return workspace.data_ptr(), workspace.numel() * workspace.element_size()
+
+
+def _out_cube(out, omega, thx, thy):
+    shape = (omega.numel(), thy.numel(), thx.numel())
+    if out is None:
+        return torch.empty(shape, dtype=torch.float64, device=omega.device)
+    _dev(out, "out")
+    if out.numel() != shape[0] * shape[1] * shape[2]:
+        raise ValueError("out has the wrong number of elements")
+    return out
+
+
+def rad_workspace_bytes(count: int, n_max: int, n_omega: int, n_thx: int, n_thy: int) -> int:
+    return int(load_library().rad_workspace_bytes(count, n_max, n_omega, n_thx, n_thy))
+
+
+def rad_classical(traj: dict, omega, thx, thy, out=None, workspace=None, stream=None):
+    """Classical cube (n_omega, n_thy, n_thx); eq. (1) with eqs. (3)-(7)."""
+    g = _grid_struct(_dev(omega, "omega"), _dev(thx, "thx"), _dev(thy, "thy"))
+    t = _traj_struct(traj)
+    out = _out_cube(out, omega, thx, thy)
+    ws, nb = _ws_args(workspace)
+    _check(load_library().rad_classical(ctypes.byref(t), ctypes.byref(g), out.data_ptr(), ws, nb,
+                                        _stream_ptr(stream)))
+    return out
+
+
+def rad_semiclassical(traj: dict, omega, thx, thy, spin: int, hbarc_over_E: float, out=None,
+                      workspace=None, stream=None):
+    """spin=0: substitution model, eq. (9); spin=1: spin-1/2 BCK, eq. (10) PAPER.md:62."""
+    g = _grid_struct(_dev(omega, "omega"), _dev(thx, "thx"), _dev(thy, "thy"))
+    t = _traj_struct(traj)
+    out = _out_cube(out, omega, thx, thy)
+    ws, nb = _ws_args(workspace)
+    _check(load_library().rad_semiclassical(ctypes.byref(t), ctypes.byref(g), int(spin), float(hbarc_over_E),
+                                            out.data_ptr(), ws, nb, _stream_ptr(stream)))
+    return out
+
+
+def rad_ensemble_sum(batch: dict, n, omega, thx, thy, model: int = CLASSICAL, hbarc_over_E=None,
+                     accumulate: bool = False, out=None, workspace=None, stream=None):
+    """Sum of the spectra of `count` trajectories.  batch: FIELDS -> (count, stride)
+    CUDA tensors; n: host int64 (count,)."""
+    ts = [_dev(batch[k], k) for k in FIELDS]
+    count, stride = ts[0].shape
+    if any(tuple(t.shape) != (count, stride) for t in ts):
+        raise ValueError("batch tensors must share one (count, stride) shape")
+    n_host = np.ascontiguousarray(n, dtype=np.int64)
+    if n_host.shape != (count,):
+        raise ValueError("n must have shape (count,)")
+    lam = None
+    if hbarc_over_E is not None:
+        lam = np.ascontiguousarray(np.broadcast_to(np.asarray(hbarc_over_E, dtype=np.float64), (count,)))
+    b = _Batch(count, stride, n_host.ctypes.data, *[t.data_ptr() for t in ts])
+    g = _grid_struct(_dev(omega, "omega"), _dev(thx, "thx"), _dev(thy, "thy"))
+    if accumulate and out is None:
+        raise ValueError("accumulate needs an existing out")
+    out = _out_cube(out, omega, thx, thy)
+    ws, nb = _ws_args(workspace)
+    _check(load_library().rad_ensemble_sum(ctypes.byref(b), ctypes.byref(g), int(model),
+                                           lam.ctypes.data if lam is not None else None,
+                                           1 if accumulate else 0, out.data_ptr(), ws, nb,
+                                           _stream_ptr(stream)))
+    return out
+
+
+def rad_angular_sum(cube, omega, thx, thy, d_solid_angle: float, theta_cut: float = 0.0, out=None,
+                    stream=None):
+    """dI/dw = sum over angles of cube * dOmega, optional collimator cut."""
+    g = _grid_struct(_dev(omega, "omega"), _dev(thx, "thx"), _dev(thy, "thy"))
+    _dev(cube, "cube")
+    if out is None:
+        out = torch.empty(omega.numel(), dtype=torch.float64, device=cube.device)
+    _check(load_library().rad_angular_sum(cube.data_ptr(), ctypes.byref(g), float(d_solid_angle),
+                                          float(theta_cut), _dev(out, "out").data_ptr(), _stream_ptr(stream)))
+    return out
+
+
+def _host(a, name: str) -> np.ndarray:
+    if isinstance(a, torch.Tensor):
+        if a.is_cuda or a.dtype != torch.float64 or not a.is_contiguous():
+            raise TypeError(f"{name}: expected a contiguous float64 CPU tensor")
+        return a.numpy()
+    a = np.asarray(a)
+    if a.dtype != np.float64 or not a.flags.c_contiguous:
+        raise TypeError(f"{name}: expected a C-contiguous float64 array")
+    return a
+
+
+def rad_eval_host(traj: dict, omega, thx, thy, model: int = CLASSICAL, hbarc_over_E: float = 0.0,
+                  out=None, stream=None):
+    """Host-buffer call: H2D, evaluate, D2H inside the C library."""
+    hs = [_host(traj[k], k) for k in FIELDS]
+    n = hs[0].shape[0]
+    w, x, y = _host(omega, "omega"), _host(thx, "thx"), _host(thy, "thy")
+    t = _Traj(n, *[h.ctypes.data for h in hs])
+    g = _Grid(w.size, x.size, y.size, w.ctypes.data, x.ctypes.data, y.ctypes.data)
+    if out is None:
+        out = np.empty((w.size, y.size, x.size), dtype=np.float64)
+    o = _host(out, "out")
+    _check(load_library().rad_eval_host(ctypes.byref(t), ctypes.byref(g), int(model), float(hbarc_over_E),
+                                        o.ctypes.data, _stream_ptr(stream)))
+    return out
+
+
+def rad_ensemble_sum_host(batch: dict, n, omega, thx, thy, model: int = CLASSICAL, hbarc_over_E=None,
+                          accumulate: bool = False, out=None, stream=None):
+    hs = [_host(batch[k], k) for k in FIELDS]
+    count, stride = hs[0].shape
+    n_host = np.ascontiguousarray(n, dtype=np.int64)
+    lam = None
+    if hbarc_over_E is not None:
+        lam = np.ascontiguousarray(np.broadcast_to(np.asarray(hbarc_over_E, dtype=np.float64), (count,)))
+    w, x, y = _host(omega, "omega"), _host(thx, "thx"), _host(thy, "thy")
+    b = _Batch(count, stride, n_host.ctypes.data, *[h.ctypes.data for h in hs])
+    g = _Grid(w.size, x.size, y.size, w.ctypes.data, x.ctypes.data, y.ctypes.data)
+    if out is None:
+        if accumulate:
+            raise ValueError("accumulate needs an existing out")
+        out = np.empty((w.size, y.size, x.size), dtype=np.float64)
+    o = _host(out, "out")
+    _check(load_library().rad_ensemble_sum_host(ctypes.byref(b), ctypes.byref(g), int(model),
+                                                lam.ctypes.data if lam is not None else None,
+                                                1 if accumulate else 0, o.ctypes.data, _stream_ptr(stream)))
+    return out
+
+
+def rad_measure_fp64_peak(millis: float = 200.0, stream=None) -> float:
+    """Measured FP64 FMA peak of the current device in FLOP/s."""
+    v = float(load_library().rad_measure_fp64_peak(float(millis), _stream_ptr(stream)))
+    if v <= 0:
+        raise RadError(-3, "rad_measure_fp64_peak failed (no CUDA device?)")
+    return v
+
+
+def rad_launch_count() -> int:
+    return int(load_library().rad_launch_count())

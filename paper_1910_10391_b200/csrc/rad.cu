@@ -1,0 +1,698 @@
+// rad.cu -- sm_100a FP64 kernels and the C ABI of include/rad.h.
+//
+// Hot path:
+//   rad_pack_kernel      a0/a1  caller SoA -> chunk records (trapezoid weights folded into the
+//                               accelerations, 1/(2 gamma^2) - dvz, chunk-relative phase terms,
+//                               double-double chunk base)                 PAPER.md:34-46 (eqs. 3-7)
+//   rad_main_kernel      a0-a5  one CTA per tile of 128 (angle, omega-group) threads x W omegas;
+//                               trajectory chunks staged by TMA bulk copies into a 3-stage
+//                               shared-memory ring; per-thread complex accumulation;
+//                               epilogue |A|^2 with the variant's coefficients
+//                                                          PAPER.md:23 (eq. 1), :56 (eq. 9), :62-68 (eqs. 10-12)
+//   rad_finalize_kernel  a6/a7  ordered reduction of time-split amplitudes / trajectory-split
+//                               spectra
+//   rad_angular_sum_kernel      sum of the cube over angles
+#include <atomic>
+#include <cmath>
+#include <cstdio>
+#include <cstring>
+#include <mutex>
+#include <vector>
+
+#include <cuda_runtime.h>
+
+#include "../../include/rad.h"
+#include "rad_device.cuh"
+
+namespace rad {
+
+constexpr int TPB = 128;     // threads per CTA: one (angle, omega-group) each
+constexpr int W = 8;         // omegas per thread (register tile)
+constexpr int STAGES = 3;    // shared-memory ring depth
+constexpr int SMEM_BYTES = STAGES * CHUNK_BYTES + STAGES * 8;
+
+enum Mode : int { MODE_DIRECT = 0, MODE_PSLICE = 1, MODE_TSPLIT = 2 };
+
+struct MainParams {
+    const double *packed;     // [count][cpt][CHUNK_DBL]
+    const int64_t *n_dev;     // samples per trajectory (device) or nullptr -> n_single
+    const double *lam_dev;    // hbar c / E per trajectory (device) or nullptr -> lam_single
+    int64_t n_single;
+    double lam_single;
+    int count, cpt;
+    const double *omega, *thx, *thy;
+    int n_omega, n_thx, n_thy;
+    int model, mode, p_slices, t_slices, accumulate;
+    double *out;
+    double *partial;
+    int64_t t_pad;            // tiles * TPB
+};
+
+// ------------------------------------------------------------------------------ pack (a0, a1)
+// P0 = t/(2 gamma^2) - dz as a double-double
+__device__ __forceinline__ dd phase_offset_dd(double gamma, double t, double dz, double &a_hi) {
+    dd g2 = two_prod(gamma, gamma);
+    dd den = {2.0 * g2.hi, 2.0 * g2.lo};
+    dd a = d_div_dd(1.0, den);                      // 1/(2 gamma^2)
+    a_hi = a.hi;
+    dd at = dd_mul_d(a, t);
+    dd s = two_sum(at.hi, -dz);
+    return fast_two_sum(s.hi, s.lo + at.lo);
+}
+
+__global__ void __launch_bounds__(256)
+rad_pack_kernel(rad_traj_batch b, const int64_t *n_dev, int64_t n_single, int cpt, double *packed) {
+    const int p = blockIdx.y;
+    const int64_t slot = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (slot >= (int64_t)cpt * CH) return;
+    const int64_t n = n_dev ? n_dev[p] : n_single;
+    const int c = (int)(slot / CH), i = (int)(slot % CH);
+    const int64_t c0 = (int64_t)c * CH;
+    if (c0 >= n) return;                              // chunk never read
+    const int64_t o = (int64_t)p * b.stride;
+    const int nvalid = (int)min((int64_t)CH, n - c0);
+    const int64_t kb = c0 + min(CH / 2, nvalid - 1);  // base sample of the chunk
+    double *chunk = packed + ((int64_t)p * cpt + c) * CHUNK_DBL;
+
+    double ab;
+    const dd P0b = phase_offset_dd(b.gamma[o + kb], b.t[o + kb], b.dz[o + kb], ab);
+    if (i == 0) {
+        chunk[0] = P0b.hi; chunk[1] = P0b.lo;
+        chunk[2] = b.t[o + kb]; chunk[3] = b.x[o + kb]; chunk[4] = b.y[o + kb];
+        chunk[5] = b.gamma[o]; chunk[6] = 0.0; chunk[7] = 0.0;
+    }
+    double *rec = chunk + HDR + i * REC;
+    const int64_t k = c0 + i;
+    if (k >= n) {                                     // zero-weight padding, q = 1
+        rec[0] = 1.0;
+#pragma unroll
+        for (int j = 1; j < REC; ++j) rec[j] = 0.0;
+        return;
+    }
+    const double tk = b.t[o + k];
+    const double w = 0.5 * (b.t[o + min(k + 1, n - 1)] - b.t[o + max(k - 1, (int64_t)0)]);
+    double ak;
+    const dd P0k = phase_offset_dd(b.gamma[o + k], tk, b.dz[o + k], ak);
+    const dd dP = dd_add(P0k, dd_neg(P0b));
+    rec[0] = ak - b.dvz[o + k];
+    rec[1] = b.vx[o + k];
+    rec[2] = b.vy[o + k];
+    rec[3] = w * b.ax[o + k];
+    rec[4] = w * b.ay[o + k];
+    rec[5] = w * b.az[o + k];
+    rec[6] = dP.hi + dP.lo;
+    rec[7] = tk - b.t[o + kb];
+    rec[8] = b.x[o + k] - b.x[o + kb];
+    rec[9] = b.y[o + k] - b.y[o + kb];
+}
+
+// ------------------------------------------------------------------------------ epilogue (a5)
+// d2I/dw dOmega (units of e^2) from A_x, A_y (and J); A_z = -(n_x A_x + n_y A_y) is the
+// transversality identity of eqs. (3)-(5).
+template <int NC>
+__device__ __forceinline__ double spectrum_value(const double (&acc)[NC], double nx, double ny,
+                                                 int model, double u, double gamma0) {
+    const double INV_4PI2 = 0.025330295910584442860969;   // 1/(4 pi^2)
+    const double azr = -(nx * acc[0] + ny * acc[2]);
+    const double azi = -(nx * acc[1] + ny * acc[3]);
+    const double S = acc[0] * acc[0] + acc[1] * acc[1] + acc[2] * acc[2] + acc[3] * acc[3]
+                   + azr * azr + azi * azi;
+    if (!(u < 1.0)) return __longlong_as_double(0x7ff8000000000000LL);   // no final state: NaN
+    if (model == RAD_CLASSICAL) return S * INV_4PI2;
+    const double e = 1.0 - u;
+    if (model == RAD_SPIN0) return e * S * INV_4PI2;
+    double J2 = 0.0;
+    if (NC == 6) J2 = acc[4] * acc[4] + acc[5] * acc[5];
+    return (0.5 * (1.0 + e * e) * S + u * u / (2.0 * gamma0 * gamma0) * J2) * INV_4PI2;
+}
+
+// ------------------------------------------------------------------------------ main (a0-a5)
+// NC = number of real accumulators per omega: 4 (A_x, A_y) or 6 (+ J, spin-1/2).
+template <int NC, int DEG>
+__global__ void __launch_bounds__(TPB)
+rad_main_kernel(const MainParams P) {
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double *ring = reinterpret_cast<double *>(smem_raw);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem_raw + STAGES * CHUNK_BYTES);
+    const int tid = threadIdx.x;
+
+    // ---- this thread's grid coordinates: flattened (omega-group, angle), angle fastest
+    const int A = P.n_thx * P.n_thy;
+    const int n_wg = (P.n_omega + W - 1) / W;
+    const int64_t T = (int64_t)n_wg * A;
+    const int64_t gid = (int64_t)blockIdx.x * TPB + tid;
+    const int64_t gc = min(gid, T - 1);
+    const int wg = (int)(gc / A), a = (int)(gc % A);
+    const double nx = P.thx[a % P.n_thx], ny = P.thy[a / P.n_thx];
+    dd h;                                             // theta^2 / 2, double-double
+    {
+        dd xx = two_prod(nx, nx), yy = two_prod(ny, ny);
+        dd s = two_sum(xx.hi, yy.hi);
+        s = fast_two_sum(s.hi, s.lo + (xx.lo + yy.lo));
+        h = {0.5 * s.hi, 0.5 * s.lo};
+    }
+    double om[W];
+#pragma unroll
+    for (int j = 0; j < W; ++j) om[j] = P.omega[min(wg * W + j, P.n_omega - 1)];
+
+    // ---- this CTA's slice of the (trajectory, chunk) axis
+    const int slice = blockIdx.y;
+    int p_begin, p_end, ts = 0;
+    if (P.mode == MODE_TSPLIT) { p_begin = slice / P.t_slices; p_end = p_begin + 1; ts = slice % P.t_slices; }
+    else { p_begin = (int)((int64_t)slice * P.count / P.p_slices);
+           p_end = (int)((int64_t)(slice + 1) * P.count / P.p_slices); }
+
+    auto chunk_range = [&](int p, int &c0, int &c1) {
+        const int64_t n = P.n_dev ? P.n_dev[p] : P.n_single;
+        const int nch = (int)((n + CH - 1) / CH);
+        if (P.mode == MODE_TSPLIT) { c0 = (int)((int64_t)ts * nch / P.t_slices);
+                                     c1 = (int)((int64_t)(ts + 1) * nch / P.t_slices); }
+        else { c0 = 0; c1 = nch; }
+    };
+
+    if (tid == 0) {
+        for (int s = 0; s < STAGES; ++s) mbar_init(&bars[s], 1);
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    // producer cursor (thread 0 only): next chunk to request
+    int pp = p_begin, pc = 0, pc1 = 0;
+    uint32_t issued = 0;
+    if (tid == 0 && pp < p_end) chunk_range(pp, pc, pc1);
+    auto produce = [&]() {                            // request one more chunk if any is left
+        while (pp < p_end && pc >= pc1) {             // move on to the next trajectory
+            ++pp;
+            if (pp < p_end) chunk_range(pp, pc, pc1);
+        }
+        if (pp >= p_end) return;
+        const int s = issued % STAGES;
+        mbar_expect_tx(&bars[s], CHUNK_BYTES);
+        tma_load_1d(ring + (size_t)s * CHUNK_DBL,
+                    P.packed + ((int64_t)pp * P.cpt + pc) * CHUNK_DBL, CHUNK_BYTES, &bars[s]);
+        ++pc;
+        ++issued;
+    };
+    if (tid == 0)
+        for (int s = 0; s < STAGES; ++s) produce();
+
+    uint32_t it = 0;                                  // chunks consumed so far by this CTA
+    double S_sum[W];
+#pragma unroll
+    for (int j = 0; j < W; ++j) S_sum[j] = 0.0;
+
+    for (int p = p_begin; p < p_end; ++p) {
+        // ---- per-trajectory constants: omega* / 2 pi as a double-double, u = hbar omega / E
+        const double lam = P.lam_dev ? P.lam_dev[p] : P.lam_single;
+        double wh[W], wl[W];
+#pragma unroll
+        for (int j = 0; j < W; ++j) {
+            dd u = two_prod(om[j], lam);
+            dd d = two_sum(1.0, -u.hi);
+            d = fast_two_sum(d.hi, d.lo - u.lo);      // 1 - u
+            dd wst = d_div_dd(om[j], d);              // omega* = omega / (1 - u)
+            dd wt = dd_mul(wst, dd{INV_2PI_HI, INV_2PI_LO});
+            wh[j] = wt.hi; wl[j] = wt.lo;
+        }
+        double acc[W][NC];
+#pragma unroll
+        for (int j = 0; j < W; ++j)
+#pragma unroll
+            for (int c = 0; c < NC; ++c) acc[j][c] = 0.0;
+        double gamma0 = 1.0;
+
+        int c0, c1;
+        chunk_range(p, c0, c1);
+        for (int c = c0; c < c1; ++c, ++it) {
+            const int s = it % STAGES;
+            mbar_wait(&bars[s], (it / STAGES) & 1);
+            const double *ck = ring + (size_t)s * CHUNK_DBL;
+
+            // ---- chunk base phase in turns, per omega, reduced to [-1/2, 1/2]  (a3, exact part)
+            double p0[W];
+            {
+                const double2 h01 = *reinterpret_cast<const double2 *>(ck);
+                const double2 h23 = *reinterpret_cast<const double2 *>(ck + 2);
+                const double2 h45 = *reinterpret_cast<const double2 *>(ck + 4);
+                gamma0 = h45.y;
+                dd psi = {h01.x, h01.y};                               // P0_b
+                psi = dd_add(psi, dd_mul_d(h, h23.x));                 // + theta^2/2 * t_b
+                psi = dd_add(psi, dd_neg(two_prod(nx, h23.y)));        // - n_x x_b
+                psi = dd_add(psi, dd_neg(two_prod(ny, h45.x)));        // - n_y y_b
+#pragma unroll
+                for (int j = 0; j < W; ++j) p0[j] = dd_frac(dd_mul(dd{wh[j], wl[j]}, psi));
+            }
+
+            // ---- samples of the chunk
+            const double *rec = ck + HDR;
+#pragma unroll 1
+            for (int k = 0; k < CH; ++k, rec += REC) {
+                const double2 r01 = *reinterpret_cast<const double2 *>(rec);       // D0, vx
+                const double2 r23 = *reinterpret_cast<const double2 *>(rec + 2);   // vy, w ax
+                const double2 r45 = *reinterpret_cast<const double2 *>(rec + 4);   // w ay, w az
+                const double2 r67 = *reinterpret_cast<const double2 *>(rec + 6);   // dP0, dt
+                const double2 r89 = *reinterpret_cast<const double2 *>(rec + 8);   // dx, dy
+                // a2: integrand geometry, independent of omega (eqs. 3, 4, 6, 12)
+                const double D = r01.x - h.hi;                 // round bracket of eqs. 3-5
+                const double ux = nx - r01.y, uy = ny - r23.x;
+                const double bx = fma(ny, uy, D);              // n_y(n_y - v_y) + D
+                const double by = fma(nx, ux, D);              // n_x(n_x - v_x) + D
+                const double q = fma(nx, ux, bx);              // eq. 6 denominator
+                const double g = inv_square(q);
+                const double s1 = fma(ny, r45.x, r45.y);       // w(az + n_y ay)
+                const double s2 = fma(nx, r23.y, r45.y);       // w(az + n_x ax)
+                const double fx = fma(s1, ux, -(bx * r23.y)) * g;      // eq. 3 (times w)
+                const double fy = fma(s2, uy, -(by * r45.x)) * g;      // eq. 4 (times w)
+                double hj = 0.0;
+                if (NC == 6) hj = fma(nx, r23.y, s1) * g;      // eq. 12 integrand (times w)
+                // eq. 7 relative to the chunk base
+                const double dpsi = fma(-ny, r89.y, fma(-nx, r89.x, fma(h.hi, r67.y, r67.x)));
+#pragma unroll
+                for (int j = 0; j < W; ++j) {
+                    double cs, sn;
+                    sincos_turns<DEG>(fma(wh[j], dpsi, p0[j]), cs, sn);            // a3
+                    acc[j][0] = fma(fx, cs, acc[j][0]);                              // a4
+                    acc[j][1] = fma(fx, sn, acc[j][1]);
+                    acc[j][2] = fma(fy, cs, acc[j][2]);
+                    acc[j][3] = fma(fy, sn, acc[j][3]);
+                    if (NC == 6) {
+                        acc[j][4] = fma(hj, cs, acc[j][4]);
+                        acc[j][5] = fma(hj, sn, acc[j][5]);
+                    }
+                }
+            }
+            __syncthreads();                          // every thread is done with stage s
+            if (tid == 0) produce();
+        }
+
+        // ---- end of this trajectory (or of this time slice of it)
+        if (P.mode == MODE_TSPLIT) {
+            double *dst = P.partial + (int64_t)slice * NC * W * P.t_pad + gid;
+#pragma unroll
+            for (int c = 0; c < NC; ++c)
+#pragma unroll
+                for (int j = 0; j < W; ++j) dst[(int64_t)(c * W + j) * P.t_pad] = acc[j][c];
+        } else {
+#pragma unroll
+            for (int j = 0; j < W; ++j)
+                S_sum[j] += spectrum_value<NC>(acc[j], nx, ny, P.model, om[j] * lam, gamma0);
+        }
+    }
+
+    if (P.mode == MODE_PSLICE) {
+        double *dst = P.partial + (int64_t)slice * W * P.t_pad + gid;
+#pragma unroll
+        for (int j = 0; j < W; ++j) dst[(int64_t)j * P.t_pad] = S_sum[j];
+    } else if (P.mode == MODE_DIRECT && gid < T) {
+#pragma unroll
+        for (int j = 0; j < W; ++j) {
+            const int iw = wg * W + j;
+            if (iw < P.n_omega) {
+                double *o = P.out + (int64_t)iw * A + a;
+                *o = P.accumulate ? *o + S_sum[j] : S_sum[j];
+            }
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------ finalize (a6, a7)
+template <int NC>
+__global__ void __launch_bounds__(TPB)
+rad_finalize_kernel(const MainParams P) {
+    const int A = P.n_thx * P.n_thy;
+    const int n_wg = (P.n_omega + W - 1) / W;
+    const int64_t T = (int64_t)n_wg * A;
+    const int64_t gid = (int64_t)blockIdx.x * TPB + threadIdx.x;
+    if (gid >= T) return;
+    const int wg = (int)(gid / A), a = (int)(gid % A);
+    const double nx = P.thx[a % P.n_thx], ny = P.thy[a / P.n_thx];
+    for (int j = 0; j < W; ++j) {
+        const int iw = wg * W + j;
+        if (iw >= P.n_omega) break;
+        const double om = P.omega[iw];
+        double total = 0.0;
+        if (P.mode == MODE_PSLICE) {
+            for (int s = 0; s < P.p_slices; ++s)                       // slices ascending
+                total += P.partial[((int64_t)s * W + j) * P.t_pad + gid];
+        } else {
+            for (int p = 0; p < P.count; ++p) {                        // trajectories ascending
+                double acc[NC];
+#pragma unroll
+                for (int c = 0; c < NC; ++c) acc[c] = 0.0;
+                for (int s = 0; s < P.t_slices; ++s) {                 // time slices ascending
+                    const double *src = P.partial + (int64_t)(p * P.t_slices + s) * NC * W * P.t_pad + gid;
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) acc[c] += src[(int64_t)(c * W + j) * P.t_pad];
+                }
+                const double lam = P.lam_dev ? P.lam_dev[p] : P.lam_single;
+                const double gamma0 = P.packed[(int64_t)p * P.cpt * CHUNK_DBL + 5];
+                total += spectrum_value<NC>(acc, nx, ny, P.model, om * lam, gamma0);
+            }
+        }
+        double *o = P.out + (int64_t)iw * A + a;
+        *o = P.accumulate ? *o + total : total;
+    }
+}
+
+// ------------------------------------------------------------------------------ angular sum
+// one CTA per omega; fixed-order tree reduction in shared memory (deterministic)
+__global__ void __launch_bounds__(256)
+rad_angular_sum_kernel(const double *cube, const double *thx, const double *thy, int n_thx, int n_thy,
+                       double d_solid, double cut2, double *spec) {
+    __shared__ double red[256];
+    const int A = n_thx * n_thy;
+    const double *src = cube + (int64_t)blockIdx.x * A;
+    double s = 0.0;
+    for (int a = threadIdx.x; a < A; a += 256) {
+        const double nx = thx[a % n_thx], ny = thy[a / n_thx];
+        if (cut2 <= 0.0 || nx * nx + ny * ny <= cut2) s += src[a];
+    }
+    red[threadIdx.x] = s;
+    __syncthreads();
+    for (int st = 128; st > 0; st >>= 1) {
+        if (threadIdx.x < st) red[threadIdx.x] += red[threadIdx.x + st];
+        __syncthreads();
+    }
+    if (threadIdx.x == 0) spec[blockIdx.x] = red[0] * d_solid;
+}
+
+// ------------------------------------------------------------------------------ FP64 peak probe
+__global__ void __launch_bounds__(256)
+rad_fma_peak_kernel(double *sink, int iters, double a, double b) {
+    double x[16];
+#pragma unroll
+    for (int i = 0; i < 16; ++i) x[i] = 1.0 + 1e-9 * (threadIdx.x + i);
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+        for (int r = 0; r < 8; ++r)
+#pragma unroll
+            for (int i = 0; i < 16; ++i) x[i] = fma(x[i], a, b);
+    }
+    double s = 0.0;
+#pragma unroll
+    for (int i = 0; i < 16; ++i) s += x[i];
+    if (s == 12345.678) sink[0] = s;      // never true; keeps the chains alive
+}
+
+// =============================================================================== host side
+static std::atomic<int64_t> g_launches{0};
+static thread_local char g_err[256] = "no CUDA error recorded";
+
+static int cuda_fail(cudaError_t e, const char *what) {
+    snprintf(g_err, sizeof g_err, "%s: %s", what, cudaGetErrorString(e));
+    return RAD_ECUDA;
+}
+#define CK(call)                                              \
+    do {                                                      \
+        cudaError_t e_ = (call);                              \
+        if (e_ != cudaSuccess) return cuda_fail(e_, #call);   \
+    } while (0)
+
+static int sm_count() {
+    static int n = 0;
+    if (n == 0) {
+        int dev = 0;
+        if (cudaGetDevice(&dev) != cudaSuccess) return 0;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) n = 0;
+    }
+    return n;
+}
+
+static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+
+// The launch plan is a pure function of the shapes (and the SM count, 148 assumed when no
+// device is visible so that rad_workspace_bytes works on a CPU-only box).
+struct Plan {
+    int cpt, tiles, p_slices, t_slices, mode;
+    int64_t t_pad;
+    size_t off_packed, off_n, off_lam, off_partial, total;
+};
+
+static Plan make_plan(int count, int64_t n_max, int n_omega, int n_thx, int n_thy, int nc) {
+    Plan pl{};
+    int sms = sm_count();
+    if (sms <= 0) sms = 148;
+    const int64_t T = (int64_t)((n_omega + W - 1) / W) * n_thx * n_thy;
+    pl.tiles = (int)((T + TPB - 1) / TPB);
+    pl.t_pad = (int64_t)pl.tiles * TPB;
+    pl.cpt = (int)((n_max + CH - 1) / CH);
+    const int target = sms * 8;                       // CTAs wanted in flight over the launch
+    pl.p_slices = 1; pl.t_slices = 1; pl.mode = MODE_DIRECT;
+    if (pl.tiles < target) {
+        const int want = (target + pl.tiles - 1) / pl.tiles;       // slices wanted per tile
+        if (count >= want) { pl.mode = MODE_PSLICE; pl.p_slices = want; }
+        else if (count > 1 || want > 1) {
+            int ts = (want + count - 1) / count;
+            ts = std::min(ts, std::max(1, pl.cpt / 2));            // >= 2 chunks per slice
+            if (ts > 1) { pl.mode = MODE_TSPLIT; pl.t_slices = ts; pl.p_slices = count; }
+            else if (count > 1) { pl.mode = MODE_PSLICE; pl.p_slices = count; }
+        }
+    }
+    size_t off = 0;
+    pl.off_packed = off; off += align_up((size_t)count * pl.cpt * CHUNK_BYTES, 256);
+    pl.off_n = off;      off += align_up((size_t)count * sizeof(int64_t), 256);
+    pl.off_lam = off;    off += align_up((size_t)count * sizeof(double), 256);
+    pl.off_partial = off;
+    if (pl.mode == MODE_PSLICE) off += align_up((size_t)pl.p_slices * W * pl.t_pad * 8, 256);
+    if (pl.mode == MODE_TSPLIT) off += align_up((size_t)count * pl.t_slices * nc * W * pl.t_pad * 8, 256);
+    pl.total = off;
+    return pl;
+}
+
+static bool grid_ok(const rad_grid *g) {
+    return g && g->n_omega > 0 && g->n_thx > 0 && g->n_thy > 0 && g->omega && g->thx && g->thy;
+}
+static bool aligned8(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 7) == 0; }
+
+template <int NC, int DEG>
+static cudaError_t launch_main(const MainParams &mp, dim3 grid, cudaStream_t st) {
+    static std::once_flag once;
+    static cudaError_t attr_err = cudaSuccess;
+    std::call_once(once, [] {
+        attr_err = cudaFuncSetAttribute(rad_main_kernel<NC, DEG>,
+                                        cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
+    });
+    if (attr_err != cudaSuccess) return attr_err;
+    rad_main_kernel<NC, DEG><<<grid, TPB, SMEM_BYTES, st>>>(mp);
+    ++g_launches;
+    return cudaGetLastError();
+}
+
+// Everything: pack, main, finalize.  All device pointers; n_host / lam_host are host arrays.
+static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const rad_grid *g, int model,
+                     const double *lam_host, int accumulate, double *out,
+                     void *workspace, size_t workspace_bytes, cudaStream_t st) {
+    if (!b || b->count < 1 || !n_host || !grid_ok(g) || !out) return RAD_EINVAL;
+    if (model < RAD_CLASSICAL || model > RAD_SPIN_HALF) return RAD_EINVAL;
+    if (model != RAD_CLASSICAL && !lam_host) return RAD_EINVAL;
+    const double *arrs[11] = {b->t, b->dz, b->x, b->y, b->vx, b->vy, b->dvz, b->ax, b->ay, b->az, b->gamma};
+    for (const double *p : arrs)
+        if (!p || !aligned8(p)) return RAD_EINVAL;
+    if (!aligned8(out) || !aligned8(g->omega) || !aligned8(g->thx) || !aligned8(g->thy)) return RAD_EINVAL;
+    int64_t n_max = 0;
+    for (int p = 0; p < b->count; ++p) {
+        if (n_host[p] < 2 || n_host[p] > b->stride) return RAD_EINVAL;
+        n_max = std::max(n_max, n_host[p]);
+        if (model != RAD_CLASSICAL && !(lam_host[p] >= 0.0)) return RAD_EDOMAIN;
+    }
+    const int nc = model == RAD_SPIN_HALF ? 6 : 4;
+    const Plan pl = make_plan(b->count, n_max, g->n_omega, g->n_thx, g->n_thy, nc);
+    if (workspace && (reinterpret_cast<uintptr_t>(workspace) & 255)) return RAD_EINVAL;
+    if (workspace && workspace_bytes < pl.total) return RAD_ENOSPACE;
+    bool own = false;
+    char *ws = static_cast<char *>(workspace);
+    if (!ws) {
+        void *pnew = nullptr;
+        CK(cudaMallocAsync(&pnew, pl.total, st));
+        ws = static_cast<char *>(pnew);
+        own = true;
+    }
+    double *packed = reinterpret_cast<double *>(ws + pl.off_packed);
+    int64_t *n_dev = nullptr;
+    double *lam_dev = nullptr;
+    if (b->count > 1) {
+        n_dev = reinterpret_cast<int64_t *>(ws + pl.off_n);
+        CK(cudaMemcpyAsync(n_dev, n_host, (size_t)b->count * sizeof(int64_t), cudaMemcpyHostToDevice, st));
+        if (model != RAD_CLASSICAL) {
+            lam_dev = reinterpret_cast<double *>(ws + pl.off_lam);
+            CK(cudaMemcpyAsync(lam_dev, lam_host, (size_t)b->count * sizeof(double), cudaMemcpyHostToDevice, st));
+        }
+    }
+    {   // a0/a1: pack
+        dim3 grid((unsigned)(((int64_t)pl.cpt * CH + 255) / 256), (unsigned)b->count);
+        rad_pack_kernel<<<grid, 256, 0, st>>>(*b, n_dev, n_host[0], pl.cpt, packed);
+        ++g_launches;
+        CK(cudaGetLastError());
+    }
+    MainParams mp{};
+    mp.packed = packed; mp.n_dev = n_dev; mp.lam_dev = lam_dev;
+    mp.n_single = n_host[0];
+    mp.lam_single = model == RAD_CLASSICAL ? 0.0 : lam_host[0];
+    mp.count = b->count; mp.cpt = pl.cpt;
+    mp.omega = g->omega; mp.thx = g->thx; mp.thy = g->thy;
+    mp.n_omega = g->n_omega; mp.n_thx = g->n_thx; mp.n_thy = g->n_thy;
+    mp.model = model; mp.mode = pl.mode; mp.p_slices = pl.p_slices; mp.t_slices = pl.t_slices;
+    mp.accumulate = accumulate ? 1 : 0;
+    mp.out = out; mp.partial = reinterpret_cast<double *>(ws + pl.off_partial);
+    mp.t_pad = pl.t_pad;
+    const int slices = pl.mode == MODE_TSPLIT ? b->count * pl.t_slices : pl.p_slices;
+    dim3 grid((unsigned)pl.tiles, (unsigned)slices);
+    cudaError_t e = nc == 6 ? launch_main<6, 6>(mp, grid, st) : launch_main<4, 6>(mp, grid, st);
+    if (e != cudaSuccess) return cuda_fail(e, "rad_main_kernel");
+    if (pl.mode != MODE_DIRECT) {
+        if (nc == 6) rad_finalize_kernel<6><<<pl.tiles, TPB, 0, st>>>(mp);
+        else rad_finalize_kernel<4><<<pl.tiles, TPB, 0, st>>>(mp);
+        ++g_launches;
+        CK(cudaGetLastError());
+    }
+    if (own) CK(cudaFreeAsync(ws, st));
+    return RAD_OK;
+}
+
+static int run_single(const rad_traj *t, const rad_grid *g, int model, double lam, double *out,
+                      void *ws, size_t ws_bytes, cudaStream_t st) {
+    if (!t) return RAD_EINVAL;
+    rad_traj_batch b{1, t->n, nullptr, t->t, t->dz, t->x, t->y, t->vx, t->vy, t->dvz,
+                     t->ax, t->ay, t->az, t->gamma};
+    const int64_t n = t->n;
+    return run_batch(&b, &n, g, model, &lam, 0, out, ws, ws_bytes, st);
+}
+
+}  // namespace rad
+
+// =============================================================================== C ABI
+using namespace rad;
+
+extern "C" {
+
+int rad_classical(const rad_traj *traj, const rad_grid *grid, double *out,
+                  void *workspace, size_t workspace_bytes, void *cuda_stream) {
+    return run_single(traj, grid, RAD_CLASSICAL, 0.0, out, workspace, workspace_bytes,
+                      static_cast<cudaStream_t>(cuda_stream));
+}
+
+int rad_semiclassical(const rad_traj *traj, const rad_grid *grid, int spin, double hbarc_over_E,
+                      double *out, void *workspace, size_t workspace_bytes, void *cuda_stream) {
+    if (spin != 0 && spin != 1) return RAD_EINVAL;
+    if (!(hbarc_over_E >= 0.0)) return RAD_EDOMAIN;
+    return run_single(traj, grid, spin == 0 ? RAD_SPIN0 : RAD_SPIN_HALF, hbarc_over_E, out,
+                      workspace, workspace_bytes, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int rad_ensemble_sum(const rad_traj_batch *batch, const rad_grid *grid, rad_model model,
+                     const double *hbarc_over_E, int accumulate, double *out,
+                     void *workspace, size_t workspace_bytes, void *cuda_stream) {
+    if (!batch) return RAD_EINVAL;
+    return run_batch(batch, batch->n, grid, (int)model, hbarc_over_E, accumulate, out,
+                     workspace, workspace_bytes, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int rad_angular_sum(const double *cube, const rad_grid *grid, double d_solid_angle, double theta_cut,
+                    double *spectrum, void *cuda_stream) {
+    if (!cube || !spectrum || !grid_ok(grid)) return RAD_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    rad_angular_sum_kernel<<<grid->n_omega, 256, 0, st>>>(
+        cube, grid->thx, grid->thy, grid->n_thx, grid->n_thy, d_solid_angle,
+        theta_cut > 0.0 ? theta_cut * theta_cut : 0.0, spectrum);
+    ++g_launches;
+    CK(cudaGetLastError());
+    return RAD_OK;
+}
+
+size_t rad_workspace_bytes(int32_t count, int64_t n_max, int32_t n_omega, int32_t n_thx, int32_t n_thy) {
+    if (count < 1 || n_max < 2 || n_omega < 1 || n_thx < 1 || n_thy < 1) return 0;
+    return make_plan(count, n_max, n_omega, n_thx, n_thy, 6).total;
+}
+
+// ---- host-buffer variants: H2D once, compute, D2H once
+int rad_ensemble_sum_host(const rad_traj_batch *b, const rad_grid *g, rad_model model,
+                          const double *hbarc_over_E, int accumulate, double *out, void *cuda_stream) {
+    if (!b || b->count < 1 || !b->n || !grid_ok(g) || !out) return RAD_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const size_t row = (size_t)b->stride, tot = row * b->count;
+    const size_t M = (size_t)g->n_omega * g->n_thx * g->n_thy;
+    const size_t ng = (size_t)g->n_omega + g->n_thx + g->n_thy;
+    const double *src[11] = {b->t, b->dz, b->x, b->y, b->vx, b->vy, b->dvz, b->ax, b->ay, b->az, b->gamma};
+    for (const double *p : src)
+        if (!p) return RAD_EINVAL;
+    double *dev = nullptr;
+    CK(cudaMallocAsync(reinterpret_cast<void **>(&dev), (11 * tot + ng + M) * sizeof(double), st));
+    const double *d[11];
+    for (int i = 0; i < 11; ++i) {
+        d[i] = dev + i * tot;
+        CK(cudaMemcpyAsync(dev + i * tot, src[i], tot * sizeof(double), cudaMemcpyHostToDevice, st));
+    }
+    double *gw = dev + 11 * tot, *gx = gw + g->n_omega, *gy = gx + g->n_thx, *dout = gy + g->n_thy;
+    CK(cudaMemcpyAsync(gw, g->omega, g->n_omega * sizeof(double), cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(gx, g->thx, g->n_thx * sizeof(double), cudaMemcpyHostToDevice, st));
+    CK(cudaMemcpyAsync(gy, g->thy, g->n_thy * sizeof(double), cudaMemcpyHostToDevice, st));
+    if (accumulate) CK(cudaMemcpyAsync(dout, out, M * sizeof(double), cudaMemcpyHostToDevice, st));
+    rad_traj_batch db{b->count, b->stride, b->n, d[0], d[1], d[2], d[3], d[4], d[5], d[6], d[7], d[8], d[9], d[10]};
+    rad_grid dg{g->n_omega, g->n_thx, g->n_thy, gw, gx, gy};
+    int rc = run_batch(&db, b->n, &dg, (int)model, hbarc_over_E, accumulate, dout, nullptr, 0, st);
+    if (rc == RAD_OK) {
+        cudaError_t e = cudaMemcpyAsync(out, dout, M * sizeof(double), cudaMemcpyDeviceToHost, st);
+        if (e != cudaSuccess) rc = cuda_fail(e, "D2H");
+    }
+    cudaFreeAsync(dev, st);
+    cudaError_t e = cudaStreamSynchronize(st);
+    if (rc == RAD_OK && e != cudaSuccess) rc = cuda_fail(e, "cudaStreamSynchronize");
+    return rc;
+}
+
+int rad_eval_host(const rad_traj *t, const rad_grid *g, rad_model model, double hbarc_over_E,
+                  double *out, void *cuda_stream) {
+    if (!t) return RAD_EINVAL;
+    if (model != RAD_CLASSICAL && !(hbarc_over_E >= 0.0)) return RAD_EDOMAIN;
+    const int64_t n = t->n;
+    rad_traj_batch b{1, t->n, &n, t->t, t->dz, t->x, t->y, t->vx, t->vy, t->dvz, t->ax, t->ay, t->az, t->gamma};
+    return rad_ensemble_sum_host(&b, g, model, &hbarc_over_E, 0, out, cuda_stream);
+}
+
+double rad_measure_fp64_peak(double millis, void *cuda_stream) {
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const int sms = sm_count();
+    if (sms <= 0) return -1.0;
+    double *sink = nullptr;
+    if (cudaMalloc(reinterpret_cast<void **>(&sink), 8) != cudaSuccess) return -1.0;
+    cudaEvent_t e0, e1;
+    cudaEventCreate(&e0); cudaEventCreate(&e1);
+    const int blocks = sms * 8, threads = 256;
+    auto run = [&](int iters) -> float {
+        cudaEventRecord(e0, st);
+        rad_fma_peak_kernel<<<blocks, threads, 0, st>>>(sink, iters, 0.999999, 1e-7);
+        ++g_launches;
+        cudaEventRecord(e1, st);
+        cudaEventSynchronize(e1);
+        float ms = 0.f;
+        cudaEventElapsedTime(&ms, e0, e1);
+        return ms;
+    };
+    run(64);                                           // warm-up
+    int iters = 512;
+    float ms = run(iters);
+    if (ms > 0.f && millis > ms) {                     // scale to the requested duration
+        iters = (int)std::min(1e8, iters * (millis / ms));
+        ms = run(iters);
+    }
+    const double flops = 2.0 * 16 * 8 * (double)iters * blocks * threads;
+    cudaEventDestroy(e0); cudaEventDestroy(e1);
+    cudaFree(sink);
+    if (cudaGetLastError() != cudaSuccess || ms <= 0.f) return -1.0;
+    return flops / (ms * 1e-3);
+}
+
+int64_t rad_launch_count(void) { return g_launches.load(); }
+
+const char *rad_strerror(int code) {
+    switch (code) {
+        case RAD_OK: return "ok";
+        case RAD_EINVAL: return "invalid argument";
+        case RAD_EDOMAIN: return "parameter outside the method's domain";
+        case RAD_ECUDA: return g_err;
+        case RAD_ENOSPACE: return "workspace too small (see rad_workspace_bytes)";
+        default: return "unknown status";
+    }
+}
+
+}  // extern "C"

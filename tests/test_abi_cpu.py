@@ -1,0 +1,103 @@
+"""CPU-side checks of the boundary: the C-ABI library builds for sm_100a, loads, exports every
+symbol include/rad.h declares, and its host logic (argument validation, workspace plan) works
+without a GPU.  No compute is attempted here."""
+import ctypes
+import re
+from pathlib import Path
+
+import numpy as np
+import pytest
+
+ROOT = Path(__file__).resolve().parent.parent
+
+
+@pytest.fixture(scope="module")
+def radlib():
+    import paper_1910_10391_b200 as rad
+    rad.build_library()
+    return rad
+
+
+def test_exports_match_header(radlib):
+    header = (ROOT / "include" / "rad.h").read_text()
+    header = re.sub(r"/\*.*?\*/", "", header, flags=re.S)
+    declared = set(re.findall(r"\b(rad_[a-z0-9_]+)\s*\(", header))
+    assert declared, "no declarations found in include/rad.h"
+    lib = ctypes.CDLL(str(radlib.library_path()))
+    missing = [n for n in sorted(declared) if not hasattr(lib, n)]
+    assert not missing, f"declared in rad.h but not exported: {missing}"
+    assert declared == set(radlib.binding.EXPORTS)
+
+
+def test_library_is_sm100a_with_tma(radlib):
+    """The fat binary holds sm_100a code and the main kernel stages chunks with TMA bulk
+    copies (SASS UBLKCP) completing on an mbarrier (SYNCS)."""
+    import subprocess
+    sass = subprocess.run(["cuobjdump", "-sass", str(radlib.library_path())], capture_output=True,
+                          text=True, check=True).stdout
+    assert "sm_100a" in sass
+    assert "UBLKCP" in sass and "SYNCS" in sass
+    assert "DFMA" in sass
+
+
+def test_strerror_and_launch_count(radlib):
+    lib = radlib.load_library()
+    assert lib.rad_strerror(0) == b"ok"
+    assert b"invalid" in lib.rad_strerror(-1)
+    assert b"workspace" in lib.rad_strerror(-4)
+    assert radlib.rad_launch_count() >= 0
+
+
+def test_workspace_plan_without_gpu(radlib):
+    """The plan is a pure function of the shapes; grows with n and count; 0 on bad shapes."""
+    f = radlib.rad_workspace_bytes
+    assert f(0, 100, 4, 4, 4) == 0 and f(1, 1, 4, 4, 4) == 0 and f(1, 100, 0, 4, 4) == 0
+    small, big = f(1, 4000, 64, 8, 8), f(1, 400000, 64, 8, 8)
+    assert 0 < small < big
+    assert f(1000, 100000, 128, 16, 16) > 8 * 1000 * 100000 * 10      # packed records: 80 B/sample
+    assert f(1, 1000000, 1024, 64, 64) < 2 * 8 * 10 * 1000000 + (1 << 20)   # direct mode: no partials
+
+
+def test_validation_happens_before_any_cuda_call(radlib):
+    """Null pointers, bad spin / model, n < 2, negative hbar c / E are rejected on the host."""
+    lib = radlib.load_library()
+    B = radlib.binding
+    buf = np.zeros(16)
+    p = buf.ctypes.data
+    grid = B._Grid(2, 2, 2, p, p, p)
+    traj = B._Traj(8, *([p] * 11))
+    out = np.zeros(8).ctypes.data
+    assert lib.rad_classical(None, ctypes.byref(grid), out, None, 0, None) == -1
+    assert lib.rad_classical(ctypes.byref(traj), None, out, None, 0, None) == -1
+    assert lib.rad_classical(ctypes.byref(traj), ctypes.byref(grid), None, None, 0, None) == -1
+    assert lib.rad_semiclassical(ctypes.byref(traj), ctypes.byref(grid), 3, 1e-15, out, None, 0, None) == -1
+    assert lib.rad_semiclassical(ctypes.byref(traj), ctypes.byref(grid), 1, -1.0, out, None, 0, None) == -2
+    assert lib.rad_classical(ctypes.byref(B._Traj(1, *([p] * 11))), ctypes.byref(grid), out, None, 0, None) == -1
+    assert lib.rad_classical(ctypes.byref(B._Traj(8, *([p] * 10 + [None]))), ctypes.byref(grid), out,
+                             None, 0, None) == -1
+    assert lib.rad_classical(ctypes.byref(traj), ctypes.byref(B._Grid(0, 2, 2, p, p, p)), out, None, 0, None) == -1
+    misaligned = B._Traj(8, *([p + 4] + [p] * 10))
+    assert lib.rad_classical(ctypes.byref(misaligned), ctypes.byref(grid), out, None, 0, None) == -1
+    n = np.array([8, 1], dtype=np.int64)
+    batch = B._Batch(2, 8, n.ctypes.data, *([p] * 11))
+    assert lib.rad_ensemble_sum(ctypes.byref(batch), ctypes.byref(grid), 0, None, 0, out, None, 0, None) == -1
+    n[1] = 9                                                          # n[p] > stride
+    assert lib.rad_ensemble_sum(ctypes.byref(batch), ctypes.byref(grid), 0, None, 0, out, None, 0, None) == -1
+    n[1] = 8
+    assert lib.rad_ensemble_sum(ctypes.byref(batch), ctypes.byref(grid), 2, None, 0, out, None, 0, None) == -1
+    assert lib.rad_angular_sum(None, ctypes.byref(grid), 1.0, 0.0, out, None) == -1
+
+
+def test_no_cpu_fallback(radlib):
+    """Without a CUDA device a compute call fails loudly with RAD_ECUDA (and the Python
+    binding refuses CPU tensors)."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    with pytest.raises(radlib.RadError) as e:
+        radlib.rad_eval_host({k: np.zeros(8) + 1.0 for k in radlib.FIELDS}, np.ones(2), np.zeros(2), np.zeros(2))
+    assert e.value.code == -3
+    with pytest.raises(TypeError):
+        radlib.rad_classical({k: torch.zeros(8, dtype=torch.float64) for k in radlib.FIELDS},
+                             torch.ones(2, dtype=torch.float64), torch.zeros(2, dtype=torch.float64),
+                             torch.zeros(2, dtype=torch.float64))

@@ -1,0 +1,283 @@
+"""GPU-vs-oracle parity (run with -m gpu on the B200 box).  Every call goes through the C ABI.
+
+Tolerance (BASELINE.json north_star, Q14): at every compared point
+|gpu - oracle| <= max(1e-9 |oracle|, 1e-12 S_max), S_max = maximum of the GPU cube;
+the GPU arg-max point is always among the compared points.
+"""
+import numpy as np
+import pytest
+
+import workloads
+
+pytestmark = pytest.mark.gpu
+
+RTOL, FLOOR = 1e-9, 1e-12
+CL, S0, SH = 0, 1, 2
+
+
+@pytest.fixture(scope="module")
+def rad():
+    import torch
+    if not torch.cuda.is_available():
+        pytest.fail("no CUDA device: the CUDA path has no CPU fallback")
+    import paper_1910_10391_b200 as rad
+    rad.build_library()
+    rad.load_library()
+    return rad
+
+
+def dev_dict(d):
+    import torch
+    return {k: torch.from_numpy(np.ascontiguousarray(v)).cuda() for k, v in d.items()}
+
+
+def dev_grid(wl):
+    import torch
+    return [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (wl.omega, wl.thx, wl.thy)]
+
+
+def assert_parity(gpu_cube, ref, idx=None, label=""):
+    """gpu_cube: full GPU cube (numpy); ref: oracle values at flat indices idx (or full cube)."""
+    flat = gpu_cube.ravel()
+    assert np.all(np.isfinite(flat)), f"{label}: non-finite GPU output"
+    s_max = flat.max()
+    got = flat if idx is None else flat[idx]
+    ref = np.asarray(ref).ravel()
+    tol = np.maximum(RTOL * np.abs(ref), FLOOR * s_max)
+    ratio = np.abs(got - ref) / tol
+    worst = int(np.argmax(ratio))
+    assert ratio[worst] <= 1.0, (f"{label}: worst |err|/tol = {ratio[worst]:.3g} at compared point {worst} "
+                                 f"(gpu {got[worst]:.17g}, oracle {ref[worst]:.17g}, S_max {s_max:.6g})")
+    return float(ratio[worst])
+
+
+def run_single(rad, wl, model, lam):
+    tr, g = dev_dict(wl.traj), dev_grid(wl)
+    if model == CL:
+        return rad.rad_classical(tr, *g).cpu().numpy()
+    return rad.rad_semiclassical(tr, *g, 0 if model == S0 else 1, lam).cpu().numpy()
+
+
+def sampled_reference(oracle_mod, wl, cube, n_random, lattice, model, lam, seed=1):
+    idx = workloads.sample_points(wl, n_random, lattice, seed=seed)
+    idx = np.unique(np.concatenate([idx, [int(np.argmax(cube))]]))      # Q14: include the arg-max
+    w, nx, ny = workloads.points_of(wl, idx)
+    return idx, oracle_mod.points(wl.traj, w, nx, ny, model, lam)
+
+
+# ------------------------------------------------------------------ small, full-grid comparisons
+def test_cfg1_full_grid(rad, oracle_mod):
+    """BASELINE.json configs[0] exactly, full grid (time-split path: 4 tiles only)."""
+    wl = workloads.make("cfg1")
+    cube = run_single(rad, wl, CL, 0.0)
+    ref = oracle_mod.grid(wl.traj, wl.omega, wl.thx, wl.thy)
+    assert_parity(cube, ref, label="cfg1")
+
+
+@pytest.mark.parametrize("model", [CL, S0, SH])
+@pytest.mark.parametrize("shape", [dict(n=2, n_omega=1, n_th=1), dict(n=129, n_omega=9, n_th=3),
+                                   dict(n=1037, n_omega=13, n_th=5)])
+def test_ragged_shapes_all_models(rad, oracle_mod, model, shape):
+    """Ragged tails everywhere: n not a multiple of the 128-sample chunk (incl. the minimum n = 2),
+    n_omega not a multiple of the 8-omega register tile, angle count not a multiple of 128."""
+    wl = workloads.make("cfg2", seed=11, **shape)
+    lam = 0.6 / wl.omega.max()
+    cube = run_single(rad, wl, model, lam)
+    ref = oracle_mod.grid(wl.traj, wl.omega, wl.thx, wl.thy, model, lam)
+    assert_parity(cube, ref, label=f"ragged {shape} model {model}")
+
+
+def test_rectangular_grid_order(rad, oracle_mod):
+    """n_thx != n_thy: cube order (i_w, i_y, i_x), x fastest (Q11)."""
+    wl = workloads.make("cfg2", n=700, n_omega=5, n_th=6, seed=5)
+    wl.thx = wl.thx[:4].copy()
+    wl.thy = (wl.thy * 0.7).copy()
+    cube = run_single(rad, wl, SH, 0.3 / wl.omega.max())
+    assert cube.shape == (5, 6, 4)
+    ref = oracle_mod.grid(wl.traj, wl.omega, wl.thx, wl.thy, SH, 0.3 / wl.omega.max())
+    assert_parity(cube, ref, label="rectangular")
+
+
+def test_nonuniform_time_and_varying_gamma(rad, oracle_mod):
+    """Trapezoid weights on a non-uniform t (Q1) and sample-wise 1/2gamma_k^2 (Q6)."""
+    wl = workloads.make("cfg2", n=900, n_omega=10, n_th=4, seed=8)
+    rng = np.random.Generator(np.random.PCG64(3))
+    t = np.sort(rng.uniform(0, wl.traj["t"][-1], 900))
+    tr = {k: np.interp(t, wl.traj["t"], v) for k, v in wl.traj.items()}
+    tr["t"] = t
+    tr["gamma"] = wl.traj["gamma"] * (1 - 1e-3 * np.linspace(0, 1, 900))
+    wl.traj = tr
+    lam = 0.5 / wl.omega.max()
+    for model in (CL, SH):
+        cube = run_single(rad, wl, model, lam)
+        ref = oracle_mod.grid(tr, wl.omega, wl.thx, wl.thy, model, lam)
+        assert_parity(cube, ref, label=f"nonuniform model {model}")
+
+
+def test_straight_line_is_exact_zero(rad):
+    """P1 on the GPU path: zero acceleration gives exactly 0, all variants."""
+    wl = workloads.make("cfg2", n=500, n_omega=8, n_th=4)
+    for k in ("ax", "ay", "az"):
+        wl.traj[k] = np.zeros(500)
+    for model in (CL, S0, SH):
+        cube = run_single(rad, wl, model, 1e-16)
+        assert np.all(cube == 0.0)
+
+
+def test_domain_u_ge_1_gives_nan_only_there(rad, oracle_mod):
+    """u = hbar w / E >= 1: NaN at those points only (include/rad.h), the rest in parity."""
+    wl = workloads.make("cfg1", n=600, n_omega=8, n_th=2)
+    lam = 1.0000001 / wl.omega[5]                 # u >= 1 from i_w = 5 on
+    cube = run_single(rad, wl, S0, lam)
+    assert np.all(np.isnan(cube[5:])) and np.all(np.isfinite(cube[:5]))
+    ref = oracle_mod.grid(wl.traj, wl.omega[:5], wl.thx, wl.thy, S0, lam)
+    assert_parity(cube[:5], ref, label="domain")
+
+
+def test_deterministic(rad):
+    wl = workloads.make("cfg2", n=2000, n_omega=16, n_th=8)
+    a = run_single(rad, wl, SH, 1e-17)
+    b = run_single(rad, wl, SH, 1e-17)
+    assert np.array_equal(a, b)
+
+
+# ------------------------------------------------------------------ launch-plan coverage
+def test_direct_mode_many_tiles(rad, oracle_mod):
+    """Grid large enough (>= 8 CTAs per SM) for the no-split path; sampled + lattice."""
+    wl = workloads.make("cfg2", n=300, n_omega=40, n_th=200, seed=21)
+    cube = run_single(rad, wl, CL, 0.0)
+    idx, ref = sampled_reference(oracle_mod, wl, cube, 3000, (5, 9, 9), CL, 0.0)
+    assert_parity(cube, ref, idx, label="direct")
+
+
+def test_workspace_argument(rad, oracle_mod):
+    """Caller-provided workspace gives the same bits as pool-allocated scratch; too small -> error."""
+    import torch
+    wl = workloads.make("cfg2", n=1500, n_omega=16, n_th=8)
+    tr, g = dev_dict(wl.traj), dev_grid(wl)
+    nb = rad.rad_workspace_bytes(1, 1500, 16, 8, 8)
+    assert nb > 0
+    ws = torch.empty(nb, dtype=torch.uint8, device="cuda")
+    a = rad.rad_classical(tr, *g, workspace=ws).cpu().numpy()
+    b = rad.rad_classical(tr, *g).cpu().numpy()
+    assert np.array_equal(a, b)
+    with pytest.raises(rad.RadError) as e:
+        rad.rad_classical(tr, *g, workspace=ws[:1024])
+    assert e.value.code == -4
+
+
+def test_invalid_arguments(rad):
+    import torch
+    wl = workloads.make("cfg1", n=100, n_omega=4, n_th=2)
+    tr, g = dev_dict(wl.traj), dev_grid(wl)
+    with pytest.raises(rad.RadError) as e:
+        rad.rad_semiclassical(tr, *g, 2, 1e-15)
+    assert e.value.code == -1
+    with pytest.raises(rad.RadError) as e:
+        rad.rad_semiclassical(tr, *g, 1, -1.0)
+    assert e.value.code == -2
+    short = {k: v[:1].contiguous() for k, v in tr.items()}
+    with pytest.raises(rad.RadError):
+        rad.rad_classical(short, *g)
+    with pytest.raises(TypeError):
+        rad.rad_classical({k: v.cpu() for k, v in tr.items()}, *g)
+    del torch
+
+
+# ------------------------------------------------------------------ ensembles
+@pytest.mark.parametrize("model", [CL, SH])
+def test_ensemble_small_ragged(rad, oracle_mod, model):
+    """Few ragged trajectories (time-split path), per-trajectory hbar c / E."""
+    we = workloads.make("cfg4", count=6, n=700, n_omega=9, n_th=5)
+    nvec = np.array([700, 512, 129, 2, 700, 333], dtype=np.int64)
+    lam = np.linspace(0.2, 0.7, 6) / we.omega.max() if model != CL else None
+    cube = rad.rad_ensemble_sum(dev_dict(we.batch), nvec, *dev_grid(we), model=model,
+                                hbarc_over_E=lam).cpu().numpy()
+    w, nx, ny = oracle_mod.grid_points(we.omega, we.thx, we.thy)
+    ref = oracle_mod.ensemble_points(we.batch, nvec, w, nx, ny, model, lam)
+    assert_parity(cube, ref, label=f"ensemble small model {model}")
+
+
+def test_ensemble_many_trajectories_and_accumulate(rad, oracle_mod):
+    """Many short trajectories on a tiny grid (trajectory-split path), then accumulate=1
+    continuing a partial ensemble (sum of section spectra)."""
+    we = workloads.make("cfg4", count=400, n=300, n_omega=8, n_th=4, seed0=900)
+    rng = np.random.Generator(np.random.PCG64(1))
+    nvec = rng.integers(2, 301, size=400).astype(np.int64)
+    b, g = dev_dict(we.batch), dev_grid(we)
+    full = rad.rad_ensemble_sum(b, nvec, *g).cpu().numpy()
+    w, nx, ny = oracle_mod.grid_points(we.omega, we.thx, we.thy)
+    ref = oracle_mod.ensemble_points(we.batch, nvec, w, nx, ny)
+    assert_parity(full, ref, label="ensemble many")
+    first = rad.rad_ensemble_sum({k: v[:150].contiguous() for k, v in b.items()}, nvec[:150], *g)
+    both = rad.rad_ensemble_sum({k: v[150:].contiguous() for k, v in b.items()}, nvec[150:], *g,
+                                accumulate=True, out=first).cpu().numpy()
+    assert_parity(both, ref, label="ensemble accumulate")
+
+
+# ------------------------------------------------------------------ host-buffer entry points
+def test_host_entry_points(rad, oracle_mod):
+    wl = workloads.make("cfg2", n=1200, n_omega=12, n_th=6)
+    lam = 0.4 / wl.omega.max()
+    cube = rad.rad_eval_host(wl.traj, wl.omega, wl.thx, wl.thy, SH, lam)
+    ref = oracle_mod.grid(wl.traj, wl.omega, wl.thx, wl.thy, SH, lam)
+    assert_parity(cube, ref, label="host single")
+    we = workloads.make("cfg4", count=4, n=500, n_omega=6, n_th=3)
+    cube = rad.rad_ensemble_sum_host(we.batch, we.n, we.omega, we.thx, we.thy)
+    w, nx, ny = oracle_mod.grid_points(we.omega, we.thx, we.thy)
+    assert_parity(cube, oracle_mod.ensemble_points(we.batch, we.n, w, nx, ny), label="host ensemble")
+
+
+# ------------------------------------------------------------------ angular sum (NEXT-1)
+def test_angular_sum(rad):
+    import torch
+    wl = workloads.make("cfg2", n=800, n_omega=12, n_th=20)
+    g = dev_grid(wl)
+    cube = rad.rad_classical(dev_dict(wl.traj), *g)
+    d_om = (wl.thx[1] - wl.thx[0]) * (wl.thy[1] - wl.thy[0])
+    cut = 2.0 / wl.meta["gamma"]
+    got = rad.rad_angular_sum(cube, *g, d_om, cut).cpu().numpy()
+    c = cube.cpu().numpy()
+    X, Y = np.meshgrid(wl.thx, wl.thy)
+    mask = X * X + Y * Y <= cut * cut
+    np.testing.assert_allclose(got, (c * mask).sum((1, 2)) * d_om, rtol=1e-13)
+    got_all = rad.rad_angular_sum(cube, *g, d_om).cpu().numpy()
+    np.testing.assert_allclose(got_all, c.sum((1, 2)) * d_om, rtol=1e-13)
+    del torch
+
+
+# ------------------------------------------------------------------ full-size configs, sampled
+def test_cfg2_full_size_sampled(rad, oracle_mod):
+    """BASELINE.json configs[1] at full size, in the launch configuration bench.py times."""
+    wl = workloads.make("cfg2")
+    cube = run_single(rad, wl, CL, 0.0)
+    idx, ref = sampled_reference(oracle_mod, wl, cube, 3000, (8, 6, 6), CL, 0.0)
+    assert_parity(cube, ref, idx, label="cfg2 full")
+
+
+def test_cfg3_full_size_sampled(rad, oracle_mod):
+    """BASELINE.json configs[2]: spin-1/2, N = 2e5, |phase| up to ~1e6 rad; 512 x 64 x 64 grid."""
+    wl = workloads.make("cfg3")
+    cube = run_single(rad, wl, SH, wl.hbarc_over_E)
+    idx, ref = sampled_reference(oracle_mod, wl, cube, 160, (4, 3, 3), SH, wl.hbarc_over_E)
+    assert_parity(cube, ref, idx, label="cfg3 full")
+
+
+def test_cfg4_reduced_ensemble_sampled(rad, oracle_mod):
+    """configs[3] shape (128 x 16 x 16 grid, batched trajectories) with 48 x 20000 samples."""
+    we = workloads.make("cfg4", count=48, n=20000)
+    cube = rad.rad_ensemble_sum(dev_dict(we.batch), we.n, *dev_grid(we)).cpu().numpy()
+    idx = workloads.sample_points(we, 100, (4, 3, 3))
+    idx = np.unique(np.concatenate([idx, [int(np.argmax(cube))]]))
+    w, nx, ny = workloads.points_of(we, idx)
+    ref = oracle_mod.ensemble_points(we.batch, we.n, w, nx, ny)
+    assert_parity(cube, ref, idx, label="cfg4 reduced")
+
+
+@pytest.mark.parametrize("model", [S0, SH])
+def test_cfg5_reduced_sampled(rad, oracle_mod, model):
+    """configs[4] (axial well, both spin variants) at N = 2e5 on the full 1024 x 64 x 64 grid."""
+    wl = workloads.make("cfg5", n=200000, model=model)
+    cube = run_single(rad, wl, model, wl.hbarc_over_E)
+    idx, ref = sampled_reference(oracle_mod, wl, cube, 120, (4, 3, 3), model, wl.hbarc_over_E)
+    assert_parity(cube, ref, idx, label=f"cfg5 model {model}")
