@@ -139,6 +139,14 @@ double rad_measure_fp64_peak(double millis, void *cuda_stream);
 /* Number of kernels the library has launched in this process (bench bookkeeping). */
 int64_t rad_launch_count(void);
 
+/* Per-kernel timing of the most recent device-buffer call (for the roofline in bench.py).
+ * rad_profile_enable(1) makes every later call record CUDA events on its stream around the
+ * pack, main and finalize kernels; rad_profile_last waits for that call's last event and
+ * writes ms[0..2] = pack, main, finalize durations in milliseconds (finalize 0 if not run).
+ * Not thread-safe across concurrent calls; off by default. */
+int rad_profile_enable(int on);
+int rad_profile_last(float *ms);
+
 /* Static text for a rad_status; for RAD_ECUDA the text of the last CUDA error seen. */
 const char *rad_strerror(int code);
 

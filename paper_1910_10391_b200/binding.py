@@ -18,7 +18,8 @@ FIELDS = ("t", "dz", "x", "y", "vx", "vy", "dvz", "ax", "ay", "az", "gamma")
 
 EXPORTS = ("rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_angular_sum",
            "rad_workspace_bytes", "rad_eval_host", "rad_ensemble_sum_host",
-           "rad_measure_fp64_peak", "rad_launch_count", "rad_strerror")
+           "rad_measure_fp64_peak", "rad_launch_count", "rad_strerror",
+           "rad_profile_enable", "rad_profile_last")
 
 _dp = ctypes.POINTER(ctypes.c_double)
 _lib = None
@@ -89,6 +90,10 @@ def load_library() -> ctypes.CDLL:
     lib.rad_measure_fp64_peak.argtypes = [dbl, vp]
     lib.rad_measure_fp64_peak.restype = dbl
     lib.rad_launch_count.restype = i64
+    lib.rad_profile_enable.argtypes = [ctypes.c_int]
+    lib.rad_profile_enable.restype = ctypes.c_int
+    lib.rad_profile_last.argtypes = [ctypes.POINTER(ctypes.c_float)]
+    lib.rad_profile_last.restype = ctypes.c_int
     lib.rad_strerror.argtypes = [ctypes.c_int]
     lib.rad_strerror.restype = ctypes.c_char_p
     for name in ("rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_angular_sum",
@@ -272,3 +277,14 @@ def rad_measure_fp64_peak(millis: float = 200.0, stream=None) -> float:
 
 def rad_launch_count() -> int:
     return int(load_library().rad_launch_count())
+
+
+def rad_profile_enable(on: bool = True) -> None:
+    _check(load_library().rad_profile_enable(1 if on else 0))
+
+
+def rad_profile_last():
+    """(pack_ms, main_ms, finalize_ms) of the most recent device-buffer call."""
+    ms = (ctypes.c_float * 3)()
+    _check(load_library().rad_profile_last(ms))
+    return float(ms[0]), float(ms[1]), float(ms[2])

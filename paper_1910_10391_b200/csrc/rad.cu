@@ -398,6 +398,25 @@ rad_fma_peak_kernel(double *sink, int iters, double a, double b) {
 static std::atomic<int64_t> g_launches{0};
 static thread_local char g_err[256] = "no CUDA error recorded";
 
+// Optional per-kernel timing of the last call (bench.py's roofline needs the main kernel's own
+// duration): events recorded on the caller's stream around pack / main / finalize.
+static std::atomic<int> g_prof{0};
+static cudaEvent_t g_ev[4];
+static bool g_ev_ready = false, g_ev_have_finalize = false;
+static std::mutex g_ev_mu;
+
+static void prof_mark(int i, cudaStream_t st) {
+    if (!g_prof.load()) return;
+    std::lock_guard<std::mutex> lk(g_ev_mu);
+    if (!g_ev_ready) {
+        for (auto &e : g_ev) cudaEventCreate(&e);
+        g_ev_ready = true;
+    }
+    cudaEventRecord(g_ev[i], st);
+    if (i == 2) g_ev_have_finalize = false;
+    if (i == 3) g_ev_have_finalize = true;
+}
+
 static int cuda_fail(cudaError_t e, const char *what) {
     snprintf(g_err, sizeof g_err, "%s: %s", what, cudaGetErrorString(e));
     return RAD_ECUDA;
@@ -518,12 +537,14 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const rad_g
             CK(cudaMemcpyAsync(lam_dev, lam_host, (size_t)b->count * sizeof(double), cudaMemcpyHostToDevice, st));
         }
     }
+    prof_mark(0, st);
     {   // a0/a1: pack
         dim3 grid((unsigned)(((int64_t)pl.cpt * CH + 255) / 256), (unsigned)b->count);
         rad_pack_kernel<<<grid, 256, 0, st>>>(*b, n_dev, n_host[0], pl.cpt, packed);
         ++g_launches;
         CK(cudaGetLastError());
     }
+    prof_mark(1, st);
     MainParams mp{};
     mp.packed = packed; mp.n_dev = n_dev; mp.lam_dev = lam_dev;
     mp.n_single = n_host[0];
@@ -539,11 +560,13 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const rad_g
     dim3 grid((unsigned)pl.tiles, (unsigned)slices);
     cudaError_t e = nc == 6 ? launch_main<6, 6>(mp, grid, st) : launch_main<4, 6>(mp, grid, st);
     if (e != cudaSuccess) return cuda_fail(e, "rad_main_kernel");
+    prof_mark(2, st);
     if (pl.mode != MODE_DIRECT) {
         if (nc == 6) rad_finalize_kernel<6><<<pl.tiles, TPB, 0, st>>>(mp);
         else rad_finalize_kernel<4><<<pl.tiles, TPB, 0, st>>>(mp);
         ++g_launches;
         CK(cudaGetLastError());
+        prof_mark(3, st);
     }
     if (own) CK(cudaFreeAsync(ws, st));
     return RAD_OK;
@@ -683,6 +706,23 @@ double rad_measure_fp64_peak(double millis, void *cuda_stream) {
 }
 
 int64_t rad_launch_count(void) { return g_launches.load(); }
+
+int rad_profile_enable(int on) {
+    g_prof.store(on ? 1 : 0);
+    return RAD_OK;
+}
+
+int rad_profile_last(float *ms) {
+    if (!ms) return RAD_EINVAL;
+    std::lock_guard<std::mutex> lk(g_ev_mu);
+    if (!g_ev_ready) return RAD_EINVAL;
+    CK(cudaEventSynchronize(g_ev[g_ev_have_finalize ? 3 : 2]));
+    CK(cudaEventElapsedTime(&ms[0], g_ev[0], g_ev[1]));
+    CK(cudaEventElapsedTime(&ms[1], g_ev[1], g_ev[2]));
+    ms[2] = 0.f;
+    if (g_ev_have_finalize) CK(cudaEventElapsedTime(&ms[2], g_ev[2], g_ev[3]));
+    return RAD_OK;
+}
 
 const char *rad_strerror(int code) {
     switch (code) {
