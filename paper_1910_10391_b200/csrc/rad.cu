@@ -26,10 +26,20 @@
 
 namespace rad {
 
+#ifndef RAD_W
+#define RAD_W 8
+#endif
+#ifndef RAD_MINB
+#define RAD_MINB 1
+#endif
+#ifndef RAD_DEG
+#define RAD_DEG 5            // polynomial set of sincos_coeffs.h: 5 = LO (1e-13, default), 6 = HI (2e-16)
+#endif
 constexpr int TPB = 128;     // threads per CTA: one (angle, omega-group) each
-constexpr int W = 8;         // omegas per thread (register tile)
+constexpr int W = RAD_W;     // omegas per thread (register tile)
 constexpr int STAGES = 3;    // shared-memory ring depth
-constexpr int SMEM_BYTES = STAGES * CHUNK_BYTES + STAGES * 8;
+constexpr int SMEM_WT = W * TPB * 16;            // per-thread omega*/2pi double-doubles, parked in smem
+constexpr int SMEM_BYTES = STAGES * CHUNK_BYTES + SMEM_WT + STAGES * 8;
 
 enum Mode : int { MODE_DIRECT = 0, MODE_PSLICE = 1, MODE_TSPLIT = 2 };
 
@@ -113,27 +123,29 @@ template <int NC>
 __device__ __forceinline__ double spectrum_value(const double (&acc)[NC], double nx, double ny,
                                                  int model, double u, double gamma0) {
     const double INV_4PI2 = 0.025330295910584442860969;   // 1/(4 pi^2)
+    // imaginary accumulators hold Im/sqrt(2) (see phasor_turns): their squares count twice
     const double azr = -(nx * acc[0] + ny * acc[2]);
     const double azi = -(nx * acc[1] + ny * acc[3]);
-    const double S = acc[0] * acc[0] + acc[1] * acc[1] + acc[2] * acc[2] + acc[3] * acc[3]
-                   + azr * azr + azi * azi;
+    const double S = acc[0] * acc[0] + acc[2] * acc[2] + azr * azr
+                   + 2.0 * (acc[1] * acc[1] + acc[3] * acc[3] + azi * azi);
     if (!(u < 1.0)) return __longlong_as_double(0x7ff8000000000000LL);   // no final state: NaN
     if (model == RAD_CLASSICAL) return S * INV_4PI2;
     const double e = 1.0 - u;
     if (model == RAD_SPIN0) return e * S * INV_4PI2;
     double J2 = 0.0;
-    if (NC == 6) J2 = acc[4] * acc[4] + acc[5] * acc[5];
+    if (NC == 6) J2 = acc[4] * acc[4] + 2.0 * acc[5] * acc[5];
     return (0.5 * (1.0 + e * e) * S + u * u / (2.0 * gamma0 * gamma0) * J2) * INV_4PI2;
 }
 
 // ------------------------------------------------------------------------------ main (a0-a5)
 // NC = number of real accumulators per omega: 4 (A_x, A_y) or 6 (+ J, spin-1/2).
 template <int NC, int DEG>
-__global__ void __launch_bounds__(TPB)
+__global__ void __launch_bounds__(TPB, RAD_MINB)
 rad_main_kernel(const MainParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *ring = reinterpret_cast<double *>(smem_raw);
-    uint64_t *bars = reinterpret_cast<uint64_t *>(smem_raw + STAGES * CHUNK_BYTES);
+    double2 *wt_sm = reinterpret_cast<double2 *>(smem_raw + STAGES * CHUNK_BYTES);   // [W][TPB]
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem_raw + STAGES * CHUNK_BYTES + SMEM_WT);
     const int tid = threadIdx.x;
 
     // ---- this thread's grid coordinates: flattened (omega-group, angle), angle fastest
@@ -151,9 +163,7 @@ rad_main_kernel(const MainParams P) {
         s = fast_two_sum(s.hi, s.lo + (xx.lo + yy.lo));
         h = {0.5 * s.hi, 0.5 * s.lo};
     }
-    double om[W];
-#pragma unroll
-    for (int j = 0; j < W; ++j) om[j] = P.omega[min(wg * W + j, P.n_omega - 1)];
+    auto omega_of = [&](int j) { return P.omega[min(wg * W + j, P.n_omega - 1)]; };
 
     // ---- this CTA's slice of the (trajectory, chunk) axis
     const int slice = blockIdx.y;
@@ -204,15 +214,18 @@ rad_main_kernel(const MainParams P) {
     for (int p = p_begin; p < p_end; ++p) {
         // ---- per-trajectory constants: omega* / 2 pi as a double-double, u = hbar omega / E
         const double lam = P.lam_dev ? P.lam_dev[p] : P.lam_single;
-        double wh[W], wl[W];
+        // (kept in shared memory: only the high words are needed inside the sample loop)
+        double wh[W];
 #pragma unroll
         for (int j = 0; j < W; ++j) {
-            dd u = two_prod(om[j], lam);
+            const double om = omega_of(j);
+            dd u = two_prod(om, lam);
             dd d = two_sum(1.0, -u.hi);
             d = fast_two_sum(d.hi, d.lo - u.lo);      // 1 - u
-            dd wst = d_div_dd(om[j], d);              // omega* = omega / (1 - u)
+            dd wst = d_div_dd(om, d);                 // omega* = omega / (1 - u)
             dd wt = dd_mul(wst, dd{INV_2PI_HI, INV_2PI_LO});
-            wh[j] = wt.hi; wl[j] = wt.lo;
+            wt_sm[j * TPB + tid] = make_double2(wt.hi, wt.lo);
+            wh[j] = wt.hi;
         }
         double acc[W][NC];
 #pragma unroll
@@ -240,7 +253,10 @@ rad_main_kernel(const MainParams P) {
                 psi = dd_add(psi, dd_neg(two_prod(nx, h23.y)));        // - n_x x_b
                 psi = dd_add(psi, dd_neg(two_prod(ny, h45.x)));        // - n_y y_b
 #pragma unroll
-                for (int j = 0; j < W; ++j) p0[j] = dd_frac(dd_mul(dd{wh[j], wl[j]}, psi));
+                for (int j = 0; j < W; ++j) {
+                    const double2 wt = wt_sm[j * TPB + tid];
+                    p0[j] = dd_frac(dd_mul(dd{wt.x, wt.y}, psi));
+                }
             }
 
             // ---- samples of the chunk
@@ -270,7 +286,7 @@ rad_main_kernel(const MainParams P) {
 #pragma unroll
                 for (int j = 0; j < W; ++j) {
                     double cs, sn;
-                    sincos_turns<DEG>(fma(wh[j], dpsi, p0[j]), cs, sn);            // a3
+                    phasor_turns<DEG>(fma(wh[j], dpsi, p0[j]), cs, sn);            // a3 (sn = sin/sqrt2)
                     acc[j][0] = fma(fx, cs, acc[j][0]);                              // a4
                     acc[j][1] = fma(fx, sn, acc[j][1]);
                     acc[j][2] = fma(fy, cs, acc[j][2]);
@@ -295,7 +311,7 @@ rad_main_kernel(const MainParams P) {
         } else {
 #pragma unroll
             for (int j = 0; j < W; ++j)
-                S_sum[j] += spectrum_value<NC>(acc[j], nx, ny, P.model, om[j] * lam, gamma0);
+                S_sum[j] += spectrum_value<NC>(acc[j], nx, ny, P.model, omega_of(j) * lam, gamma0);
         }
     }
 
@@ -386,7 +402,7 @@ rad_fma_peak_kernel(double *sink, int iters, double a, double b) {
 #pragma unroll
         for (int r = 0; r < 8; ++r)
 #pragma unroll
-            for (int i = 0; i < 16; ++i) x[i] = fma(x[i], a, b);
+            for (int i = 0; i < 16; ++i) x[i] = fma(x[i], a, x[(i + 1) & 15]);   // two register operands + one: no bank stall
     }
     double s = 0.0;
 #pragma unroll
@@ -558,7 +574,7 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const rad_g
     mp.t_pad = pl.t_pad;
     const int slices = pl.mode == MODE_TSPLIT ? b->count * pl.t_slices : pl.p_slices;
     dim3 grid((unsigned)pl.tiles, (unsigned)slices);
-    cudaError_t e = nc == 6 ? launch_main<6, 6>(mp, grid, st) : launch_main<4, 6>(mp, grid, st);
+    cudaError_t e = nc == 6 ? launch_main<6, RAD_DEG>(mp, grid, st) : launch_main<4, RAD_DEG>(mp, grid, st);
     if (e != cudaSuccess) return cuda_fail(e, "rad_main_kernel");
     prof_mark(2, st);
     if (pl.mode != MODE_DIRECT) {
@@ -683,7 +699,7 @@ double rad_measure_fp64_peak(double millis, void *cuda_stream) {
     const int blocks = sms * 8, threads = 256;
     auto run = [&](int iters) -> float {
         cudaEventRecord(e0, st);
-        rad_fma_peak_kernel<<<blocks, threads, 0, st>>>(sink, iters, 0.999999, 1e-7);
+        rad_fma_peak_kernel<<<blocks, threads, 0, st>>>(sink, iters, -0.4999, 1e-7);
         ++g_launches;
         cudaEventRecord(e1, st);
         cudaEventSynchronize(e1);

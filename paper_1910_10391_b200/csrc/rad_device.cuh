@@ -80,45 +80,58 @@ __device__ __forceinline__ double dd_frac(dd a) {
     return (a.hi - k) + a.lo;
 }
 
-// ------------------------------------------------------------------ sincos in turns
-// cos(2 pi p), sin(2 pi p) for |p| < 2^48.  Reduction is exact: k = nearest multiple of
-// 1/4 (magic-number add), r = p - k in [-1/8, 1/8]; two Horner polynomials in r^2; the
-// quadrant is applied with integer selects / sign-bit xors (no FP64 pipe work).
+// ------------------------------------------------------------------ phasor of a phase in turns
+// For |p| < 2^50 turns returns  c = cos(2 pi p)  and  s = sin(2 pi p) / sqrt(2).
+// Reduction is exact: k = rint(p) by the magic-number add, r = p - k in [-1/2, 1/2].
+// Then a = sqrt(2) sin(pi r/2) and b = 2 cos(pi r/2) by two Horner polynomials in r^2, and two
+// angle doublings written so that every step is one FP64 instruction:
+//     cos(pi r) = 1 - a^2            sqrt(2) sin(pi r) = a b =: S2
+//     cos(2 pi r) = 1 - S2^2         sin(2 pi r)/sqrt(2) = S2 cos(pi r)
+// No quadrant logic, no selects, no integer instructions: on B200 an ALU instruction issued
+// between DFMAs costs FP64 issue time, so the four extra FP64
+// instructions are cheaper than the ~10 integer ones of a swap/sign scheme.  The 1/sqrt(2)
+// on the sine is carried by the imaginary accumulators and undone in the epilogue.
+// Coefficients live in constant memory so that every Horner step is one DFMA with a
+// constant-bank operand (no UMOV / MOV to materialise 64-bit immediates in the loop).
+__constant__ double SC_S6[7] = RAD_SC_HI_S;
+__constant__ double SC_C6[7] = RAD_SC_HI_C;
+__constant__ double SC_S5[6] = RAD_SC_LO_S;
+__constant__ double SC_C5[6] = RAD_SC_LO_C;
+
 template <int DEG>
 __device__ __forceinline__ void sincos_poly(double z, double &ps, double &pc);
 template <>
 __device__ __forceinline__ void sincos_poly<6>(double z, double &ps, double &pc) {
-    constexpr double S[7] = RAD_SC_HI_S;
-    constexpr double C[7] = RAD_SC_HI_C;
-    ps = S[6]; pc = C[6];
+    ps = SC_S6[6]; pc = SC_C6[6];
 #pragma unroll
-    for (int i = 5; i >= 0; --i) { ps = fma(ps, z, S[i]); pc = fma(pc, z, C[i]); }
+    for (int i = 5; i >= 0; --i) { ps = fma(ps, z, SC_S6[i]); pc = fma(pc, z, SC_C6[i]); }
 }
 template <>
 __device__ __forceinline__ void sincos_poly<5>(double z, double &ps, double &pc) {
-    constexpr double S[6] = RAD_SC_LO_S;
-    constexpr double C[6] = RAD_SC_LO_C;
-    ps = S[5]; pc = C[5];
+    ps = SC_S5[5]; pc = SC_C5[5];
 #pragma unroll
-    for (int i = 4; i >= 0; --i) { ps = fma(ps, z, S[i]); pc = fma(pc, z, C[i]); }
+    for (int i = 4; i >= 0; --i) { ps = fma(ps, z, SC_S5[i]); pc = fma(pc, z, SC_C5[i]); }
+}
+// sine of set 5 (4.7e-15) with cosine of set 6 (2e-16): one DFMA less than <6>
+template <>
+__device__ __forceinline__ void sincos_poly<56>(double z, double &ps, double &pc) {
+    ps = SC_S5[5]; pc = fma(SC_C6[6], z, SC_C6[5]);
+#pragma unroll
+    for (int i = 4; i >= 0; --i) { ps = fma(ps, z, SC_S5[i]); pc = fma(pc, z, SC_C6[i]); }
 }
 
 template <int DEG>
-__device__ __forceinline__ void sincos_turns(double p, double &c_out, double &s_out) {
-    const double MAGIC = 1688849860263936.0;         // 1.5 * 2^50: ulp = 1/4
-    double kq = p + MAGIC;
-    int q = __double2loint(kq);                      // low bits = quadrant count
-    double r = p - (kq - MAGIC);
+__device__ __forceinline__ void phasor_turns(double p, double &c_out, double &s_out) {
+    const double M52 = 6755399441055744.0;           // 1.5 * 2^52: ulp = 1
+    const double kq = p + M52;
+    const double r = p - (kq - M52);
     double ps, pc;
     sincos_poly<DEG>(r * r, ps, pc);
-    double sn = r * ps;
-    bool odd = q & 1;
-    double cs = odd ? sn : pc;
-    double ss = odd ? pc : sn;
-    int chi = __double2hiint(cs) ^ (((q + 1) << 30) & 0x80000000);
-    int shi = __double2hiint(ss) ^ ((q << 30) & 0x80000000);
-    c_out = __hiloint2double(chi, __double2loint(cs));
-    s_out = __hiloint2double(shi, __double2loint(ss));
+    const double a = r * ps;
+    const double c2 = fma(-a, a, 1.0);
+    const double s2 = a * pc;
+    c_out = fma(-s2, s2, 1.0);
+    s_out = s2 * c2;
 }
 
 // 1/(x*x) for x > 0: hardware seed (2^-23) + one cubic step (-> 2^-69) on x^2.
