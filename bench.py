@@ -35,9 +35,12 @@ sys.path.insert(0, str(ROOT))
 
 METRIC = "fp64_radiation_integral_evals_per_s"
 UNIT = "evals/s"
-# algorithmic FP64 flops per eval (52-60; low end for
-# the 4-accumulator variants, +4 for spin-1/2's J accumulator).
-FLOPS_PER_EVAL = {0: 52.0, 1: 52.0, 2: 56.0}
+# algorithmic FP64 flops per eval, enumerated there operation by operation
+# (phase 2, exact range reduction 3, quarter-angle polynomials 21, two doublings 7, complex
+# accumulation 8 [+4 for spin-1/2's J], integrand geometry 34 [37] per 8 omegas) and checked
+# against ncu's 2*DFMA + DMUL + DADD count (45.6 on cfg2).  SURVEY.md 8(d) estimated 52-60.
+FLOPS_PER_EVAL = {0: 45.25, 1: 45.25, 2: 49.6}
+FP64_INSTR_PER_EVAL = {0: 26.6, 1: 26.6, 2: 28.9}
 FP64_SPEC_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # 148 SM x 64 FMA lanes x 2 x 1.965 GHz
 
 
@@ -50,21 +53,24 @@ def parse():
     ap.add_argument("--workload", default="cfg2")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--cfg4-count", type=int, default=1000)
+    ap.add_argument("--spin", choices=["0", "1/2"], default="1/2",
+                    help="semi-classical variant of cfg3 / cfg5 (BASELINE.json configs[4] asks for both)")
     return ap.parse_args()
 
 
-def make_workload(name: str, rank: int, cfg4_count: int):
+def make_workload(name: str, rank: int, cfg4_count: int, spin: str = "1/2"):
     import workloads
+    model = workloads.SPIN0 if spin == "0" else workloads.SPIN_HALF
     if name == "cfg2":
         return workloads.make("cfg2", seed=2 + 1000 * rank)
     if name == "cfg1":
         return workloads.make("cfg1")
     if name == "cfg3":
-        return workloads.make("cfg3", seed=3 + 1000 * rank)
+        return workloads.make("cfg3", seed=3 + 1000 * rank, model=model)
     if name == "cfg4":
         return workloads.make("cfg4", count=cfg4_count, seed0=4000 + 100000 * rank)
     if name == "cfg5":
-        return workloads.make("cfg5", seed=5 + 1000 * rank)
+        return workloads.make("cfg5", seed=5 + 1000 * rank, model=model)
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -165,7 +171,7 @@ def run_reference(args):
         return 0
     import oracle
     oracle.build_all()
-    wl = make_workload(args.workload, 0, min(args.cfg4_count, 8))
+    wl = make_workload(args.workload, 0, min(args.cfg4_count, 8), args.spin)
     samples = int(np.sum(wl.n)) if wl.batch is not None else len(wl.traj["t"])
     cores = oracle.threads("f64")
     budget_s = 90.0 / max(1, args.steps + args.warmup)
@@ -209,7 +215,7 @@ def run_b200(args):
     rad.build_library()
     rad.load_library()
 
-    wl = make_workload(args.workload, rank, args.cfg4_count)
+    wl = make_workload(args.workload, rank, args.cfg4_count, args.spin)
     model, lam = wl.model, wl.hbarc_over_E
     grid = [torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (wl.omega, wl.thx, wl.thy)]
     src = wl.batch if wl.batch is not None else wl.traj
@@ -322,7 +328,9 @@ def run_b200(args):
                          "frac": achieved / peak, "traffic": None,
                          "peak_kind": "FP64 FMA microbenchmark measured in this run (rad_measure_fp64_peak)",
                          "peak_spec": FP64_SPEC_TFLOPS, "frac_of_spec": achieved / 1e12 / FP64_SPEC_TFLOPS,
-                         "flops_per_eval": FLOPS_PER_EVAL[model], "main_kernel_ms": main_s * 1e3,
+                         "flops_per_eval": FLOPS_PER_EVAL[model],
+                         "fp64_issue_frac": FP64_INSTR_PER_EVAL[model] * evals_step / main_s / (peak / 2.0),
+                         "main_kernel_ms": main_s * 1e3,
                          "main_kernel_share_of_step": main_s * 1e3 / (total_ms / args.steps)},
         }
         if not args.no_cpu_baseline and world == 1:

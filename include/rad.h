@@ -116,6 +116,13 @@ int rad_ensemble_sum(const rad_traj_batch *batch, const rad_grid *grid, rad_mode
 int rad_angular_sum(const double *cube, const rad_grid *grid, double d_solid_angle,
                     double theta_cut, double *spectrum, void *cuda_stream);
 
+/* out[i] (+)= cubes[0*m + i] + cubes[1*m + i] + ... + cubes[(count-1)*m + i], added in that
+ * order (fixed order: deterministic).  Combines the partial cubes of ensemble shards -- other
+ * GPUs' (after an all-gather) or successive batches' -- into the ensemble sum of PAPER.md:75,
+ * 149.  cubes: count*m doubles, out: m doubles, both DEVICE; out must not overlap cubes. */
+int rad_sum_cubes(const double *cubes, int32_t count, int64_t m, int accumulate, double *out,
+                  void *cuda_stream);
+
 /* Scratch needed by any call above for `count` trajectories of at most n_max samples on a
  * grid of the given shape (count = 1 for the single-trajectory calls).  0 on bad input. */
 size_t rad_workspace_bytes(int32_t count, int64_t n_max,

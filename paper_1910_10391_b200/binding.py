@@ -16,7 +16,7 @@ _SO = _PKG / "librad_b200.so"
 CLASSICAL, SPIN0, SPIN_HALF = 0, 1, 2
 FIELDS = ("t", "dz", "x", "y", "vx", "vy", "dvz", "ax", "ay", "az", "gamma")
 
-EXPORTS = ("rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_angular_sum",
+EXPORTS = ("rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_angular_sum", "rad_sum_cubes",
            "rad_workspace_bytes", "rad_eval_host", "rad_ensemble_sum_host",
            "rad_measure_fp64_peak", "rad_launch_count", "rad_strerror",
            "rad_profile_enable", "rad_profile_last")
@@ -82,6 +82,7 @@ def load_library() -> ctypes.CDLL:
     lib.rad_ensemble_sum.argtypes = [ctypes.POINTER(_Batch), ctypes.POINTER(_Grid), ctypes.c_int, vp,
                                      ctypes.c_int, vp, vp, sz, vp]
     lib.rad_angular_sum.argtypes = [vp, ctypes.POINTER(_Grid), dbl, dbl, vp, vp]
+    lib.rad_sum_cubes.argtypes = [vp, i32, i64, ctypes.c_int, vp, vp]
     lib.rad_workspace_bytes.argtypes = [i32, i64, i32, i32, i32]
     lib.rad_workspace_bytes.restype = sz
     lib.rad_eval_host.argtypes = [ctypes.POINTER(_Traj), ctypes.POINTER(_Grid), ctypes.c_int, dbl, vp, vp]
@@ -97,7 +98,7 @@ def load_library() -> ctypes.CDLL:
     lib.rad_strerror.argtypes = [ctypes.c_int]
     lib.rad_strerror.restype = ctypes.c_char_p
     for name in ("rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_angular_sum",
-                 "rad_eval_host", "rad_ensemble_sum_host"):
+                 "rad_sum_cubes", "rad_eval_host", "rad_ensemble_sum_host"):
         getattr(lib, name).restype = ctypes.c_int
     _lib = lib
     return lib
@@ -215,6 +216,21 @@ def rad_angular_sum(cube, omega, thx, thy, d_solid_angle: float, theta_cut: floa
         out = torch.empty(omega.numel(), dtype=torch.float64, device=cube.device)
     _check(load_library().rad_angular_sum(cube.data_ptr(), ctypes.byref(g), float(d_solid_angle),
                                           float(theta_cut), _dev(out, "out").data_ptr(), _stream_ptr(stream)))
+    return out
+
+
+def rad_sum_cubes(cubes, accumulate: bool = False, out=None, stream=None):
+    """Sum of ``cubes[c]`` over the leading axis in ascending order (ensemble shards)."""
+    _dev(cubes, "cubes")
+    count, m = cubes.shape[0], cubes[0].numel()
+    if out is None:
+        if accumulate:
+            raise ValueError("accumulate needs an existing out")
+        out = torch.empty(cubes.shape[1:], dtype=torch.float64, device=cubes.device)
+    if _dev(out, "out").numel() != m:
+        raise ValueError("out has the wrong number of elements")
+    _check(load_library().rad_sum_cubes(cubes.data_ptr(), count, m, 1 if accumulate else 0, out.data_ptr(),
+                                        _stream_ptr(stream)))
     return out
 
 

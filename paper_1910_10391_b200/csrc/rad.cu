@@ -392,6 +392,17 @@ rad_angular_sum_kernel(const double *cube, const double *thx, const double *thy,
     if (threadIdx.x == 0) spec[blockIdx.x] = red[0] * d_solid;
 }
 
+// ------------------------------------------------------------------------------ ordered cube sum
+// out[m] (+)= cubes[0][m] + cubes[1][m] + ... in ascending index order (a7 across shards)
+__global__ void __launch_bounds__(256)
+rad_sum_cubes_kernel(const double *cubes, int count, int64_t m, int accumulate, double *out) {
+    const int64_t i = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= m) return;
+    double s = accumulate ? out[i] : 0.0;
+    for (int c = 0; c < count; ++c) s += cubes[(int64_t)c * m + i];
+    out[i] = s;
+}
+
 // ------------------------------------------------------------------------------ FP64 peak probe
 __global__ void __launch_bounds__(256)
 rad_fma_peak_kernel(double *sink, int iters, double a, double b) {
@@ -633,6 +644,16 @@ int rad_angular_sum(const double *cube, const rad_grid *grid, double d_solid_ang
     rad_angular_sum_kernel<<<grid->n_omega, 256, 0, st>>>(
         cube, grid->thx, grid->thy, grid->n_thx, grid->n_thy, d_solid_angle,
         theta_cut > 0.0 ? theta_cut * theta_cut : 0.0, spectrum);
+    ++g_launches;
+    CK(cudaGetLastError());
+    return RAD_OK;
+}
+
+int rad_sum_cubes(const double *cubes, int32_t count, int64_t m, int accumulate, double *out,
+                  void *cuda_stream) {
+    if (!cubes || !out || count < 1 || m < 1 || !aligned8(cubes) || !aligned8(out)) return RAD_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    rad_sum_cubes_kernel<<<(unsigned)((m + 255) / 256), 256, 0, st>>>(cubes, count, m, accumulate ? 1 : 0, out);
     ++g_launches;
     CK(cudaGetLastError());
     return RAD_OK;

@@ -281,3 +281,46 @@ def test_cfg5_reduced_sampled(rad, oracle_mod, model):
     cube = run_single(rad, wl, model, wl.hbarc_over_E)
     idx, ref = sampled_reference(oracle_mod, wl, cube, 120, (4, 3, 3), model, wl.hbarc_over_E)
     assert_parity(cube, ref, idx, label=f"cfg5 model {model}")
+
+
+# ------------------------------------------------------------------ sharding on one GPU
+def test_sum_cubes_ordered(rad):
+    import torch
+    rng = np.random.Generator(np.random.PCG64(9))
+    parts = rng.standard_normal((5, 7, 3, 11)) * 10.0 ** rng.integers(-8, 8, size=(5, 1, 1, 1))
+    d = torch.from_numpy(parts).cuda()
+    got = rad.rad_sum_cubes(d).cpu().numpy()
+    want = parts[0].copy()
+    for c in range(1, 5):
+        want += parts[c]                                   # same order => same bits
+    assert np.array_equal(got, want)
+    again = rad.rad_sum_cubes(d, accumulate=True, out=torch.from_numpy(want).cuda()).cpu().numpy()
+    acc = want.copy()
+    for c in range(5):
+        acc += parts[c]
+    assert np.array_equal(again, acc)
+
+
+def test_shards_run_sequentially_equal_unsharded(rad, oracle_mod):
+    """Grid shards (omega slabs) reproduce the unsharded cube bit for bit when the launch plan is the
+    same per point, and within tolerance otherwise; ensemble shards + rad_sum_cubes match the oracle."""
+    import torch
+    from paper_1910_10391_b200.sharding import shard_range
+    wl = workloads.make("cfg2", n=900, n_omega=11, n_th=6, seed=14)
+    tr, g = dev_dict(wl.traj), dev_grid(wl)
+    ref = oracle_mod.grid(wl.traj, wl.omega, wl.thx, wl.thy)
+    slabs = []
+    for r in range(3):
+        lo, hi = shard_range(11, r, 3)
+        slabs.append(rad.rad_classical(tr, g[0][lo:hi].contiguous(), g[1], g[2]))
+    assert_parity(torch.cat(slabs).cpu().numpy(), ref, label="grid shards")
+
+    we = workloads.make("cfg4", count=7, n=400, n_omega=6, n_th=4, seed0=50)
+    b, ge = dev_dict(we.batch), dev_grid(we)
+    parts = []
+    for r in range(3):
+        lo, hi = shard_range(7, r, 3)
+        parts.append(rad.rad_ensemble_sum({k: v[lo:hi].contiguous() for k, v in b.items()}, we.n[lo:hi], *ge))
+    total = rad.rad_sum_cubes(torch.stack(parts)).cpu().numpy()
+    w, nx, ny = oracle_mod.grid_points(we.omega, we.thx, we.thy)
+    assert_parity(total, oracle_mod.ensemble_points(we.batch, we.n, w, nx, ny), label="ensemble shards")
