@@ -4,6 +4,8 @@ Tolerance (BASELINE.json north_star, Q14): at every compared point
 |gpu - oracle| <= max(1e-9 |oracle|, 1e-12 S_max), S_max = maximum of the GPU cube;
 the GPU arg-max point is always among the compared points.
 """
+import os
+
 import numpy as np
 import pytest
 
@@ -46,6 +48,10 @@ def assert_parity(gpu_cube, ref, idx=None, label=""):
     tol = np.maximum(RTOL * np.abs(ref), FLOOR * s_max)
     ratio = np.abs(got - ref) / tol
     worst = int(np.argmax(ratio))
+    if os.environ.get("RAD_PARITY_LOG"):                     # optional record for profiles/ 
+        with open(os.environ["RAD_PARITY_LOG"], "a") as f:
+            f.write(f"{label}\t{len(ref)} points\tworst |err|/tol = {ratio[worst]:.3e}\t"
+                    f"max rel err = {np.max(np.abs(got - ref) / np.maximum(np.abs(ref), 1e-300)):.3e}\n")
     assert ratio[worst] <= 1.0, (f"{label}: worst |err|/tol = {ratio[worst]:.3g} at compared point {worst} "
                                  f"(gpu {got[worst]:.17g}, oracle {ref[worst]:.17g}, S_max {s_max:.6g})")
     return float(ratio[worst])
