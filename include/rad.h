@@ -146,6 +146,13 @@ double rad_measure_fp64_peak(double millis, void *cuda_stream);
 /* Number of kernels the library has launched in this process (bench bookkeeping). */
 int64_t rad_launch_count(void);
 
+/* Which main kernel later calls use.  0 (default): chosen from the grid shape -- the separable-phasor
+ * kernel (e^{i w psi} = T(w, n_x) Y(w, n_y) on a tensor grid, exact because theta^2 = n_x^2 + n_y^2,
+ * eq. (7)) when padding the grid to its 16 x 16 x 16 (spin-1/2: 16 x 16 x 8) point tiles
+ * wastes less than half of the work, else the direct kernel (one phasor per eval).  1: always direct,
+ * 2: always separable.  Both meet the same tolerance; process-wide; RAD_EINVAL on other values. */
+int rad_set_kernel(int choice);
+
 /* Per-kernel timing of the most recent device-buffer call (for the roofline in bench.py).
  * rad_profile_enable(1) makes every later call record CUDA events on its stream around the
  * pack, main and finalize kernels; rad_profile_last waits for that call's last event and

@@ -19,7 +19,7 @@ FIELDS = ("t", "dz", "x", "y", "vx", "vy", "dvz", "ax", "ay", "az", "gamma")
 EXPORTS = ("rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_angular_sum", "rad_sum_cubes",
            "rad_workspace_bytes", "rad_eval_host", "rad_ensemble_sum_host",
            "rad_measure_fp64_peak", "rad_launch_count", "rad_strerror",
-           "rad_profile_enable", "rad_profile_last")
+           "rad_profile_enable", "rad_profile_last", "rad_set_kernel")
 
 _dp = ctypes.POINTER(ctypes.c_double)
 _lib = None
@@ -52,7 +52,7 @@ def library_path() -> Path:
 def build_library(force: bool = False, verbose: bool = False) -> Path:
     """Compile csrc/rad.cu for sm_100a into the in-tree shared library (nvcc cross-compiles
     without a GPU)."""
-    srcs = [_SRC / "rad.cu", _SRC / "rad_device.cuh", _SRC / "sincos_coeffs.h",
+    srcs = [_SRC / "rad.cu", _SRC / "rad_device.cuh", _SRC / "rad_sep.cuh", _SRC / "sincos_coeffs.h",
             _PKG.parent / "include" / "rad.h"]
     if not force and _SO.exists() and all(_SO.stat().st_mtime >= s.stat().st_mtime for s in srcs):
         return _SO
@@ -293,6 +293,14 @@ def rad_measure_fp64_peak(millis: float = 200.0, stream=None) -> float:
 
 def rad_launch_count() -> int:
     return int(load_library().rad_launch_count())
+
+
+def rad_set_kernel(choice: int = 0) -> None:
+    """0: choose by grid shape (default), 1: direct-phasor kernel, 2: separable-phasor kernel."""
+    lib = load_library()
+    lib.rad_set_kernel.argtypes = [ctypes.c_int]
+    lib.rad_set_kernel.restype = ctypes.c_int
+    _check(lib.rad_set_kernel(int(choice)))
 
 
 def rad_profile_enable(on: bool = True) -> None:

@@ -58,6 +58,10 @@ struct MainParams {
     int64_t t_pad;            // tiles * TPB
 };
 
+}  // namespace rad
+#include "rad_sep.cuh"
+namespace rad {
+
 // ------------------------------------------------------------------------------ pack (a0, a1)
 // P0 = t/(2 gamma^2) - dz as a double-double
 __device__ __forceinline__ dd phase_offset_dd(double gamma, double t, double dz, double &a_hi) {
@@ -469,29 +473,74 @@ static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 // The launch plan is a pure function of the shapes (and the SM count, 148 assumed when no
 // device is visible so that rad_workspace_bytes works on a CPU-only box).
 struct Plan {
+    int kernel;               // 0: rad_main_kernel (one phasor per eval), 1: rad_sep_kernel (separable phasor)
     int cpt, tiles, p_slices, t_slices, mode;
     int64_t t_pad;
     size_t off_packed, off_n, off_lam, off_partial, total;
 };
 
-static Plan make_plan(int count, int64_t n_max, int n_omega, int n_thx, int n_thy, int nc) {
+static std::atomic<int> g_kernel_choice{0};          // rad_set_kernel: 0 auto, 1 direct, 2 separable
+
+// The separable kernel works on tiles of 16 omega x 16 n_x x (16 or 8) n_y points: use it when padding
+// the grid to whole tiles wastes less than half of the work (it needs about half the FP64
+// instructions per eval of the direct kernel).
+static int choose_kernel(int n_omega, int n_thx, int n_thy, int nc) {
+    const int choice = g_kernel_choice.load();
+    if (choice == 1) return 0;
+    if (choice == 2) return 1;
+    const int ty = nc == 6 ? 8 : 16;
+    const double padded = (double)((n_omega + 15) / 16 * 16) * ((n_thx + 15) / 16 * 16) * ((n_thy + ty - 1) / ty * ty);
+    return (double)n_omega * n_thx * n_thy >= 0.5 * padded ? 1 : 0;
+}
+
+static Plan make_plan(int count, int64_t n_max, int n_omega, int n_thx, int n_thy, int nc, int kernel) {
     Plan pl{};
+    pl.kernel = kernel;
     int sms = sm_count();
     if (sms <= 0) sms = 148;
-    const int64_t T = (int64_t)((n_omega + W - 1) / W) * n_thx * n_thy;
-    pl.tiles = (int)((T + TPB - 1) / TPB);
-    pl.t_pad = (int64_t)pl.tiles * TPB;
     pl.cpt = (int)((n_max + CH - 1) / CH);
-    const int target = sms * 8;                       // CTAs wanted in flight over the launch
     pl.p_slices = 1; pl.t_slices = 1; pl.mode = MODE_DIRECT;
-    if (pl.tiles < target) {
-        const int want = (target + pl.tiles - 1) / pl.tiles;       // slices wanted per tile
-        if (count >= want) { pl.mode = MODE_PSLICE; pl.p_slices = want; }
-        else if (count > 1 || want > 1) {
-            int ts = (want + count - 1) / count;
-            ts = std::min(ts, std::max(1, pl.cpt / 2));            // >= 2 chunks per slice
-            if (ts > 1) { pl.mode = MODE_TSPLIT; pl.t_slices = ts; pl.p_slices = count; }
-            else if (count > 1) { pl.mode = MODE_PSLICE; pl.p_slices = count; }
+    size_t per_thread_p, per_thread_t;                // partial doubles per thread and slice
+    if (kernel == 0) {
+        const int64_t T = (int64_t)((n_omega + W - 1) / W) * n_thx * n_thy;
+        pl.tiles = (int)((T + TPB - 1) / TPB);
+        pl.t_pad = (int64_t)pl.tiles * TPB;
+        per_thread_p = W; per_thread_t = (size_t)nc * W;
+        const int target = sms * 8;                   // CTAs wanted in flight over the launch
+        if (pl.tiles < target) {
+            const int want = (target + pl.tiles - 1) / pl.tiles;       // slices wanted per tile
+            if (count >= want) { pl.mode = MODE_PSLICE; pl.p_slices = want; }
+            else if (count > 1 || want > 1) {
+                int ts = (want + count - 1) / count;
+                ts = std::min(ts, std::max(1, pl.cpt / 2));            // >= 2 chunks per slice
+                if (ts > 1) { pl.mode = MODE_TSPLIT; pl.t_slices = ts; pl.p_slices = count; }
+                else if (count > 1) { pl.mode = MODE_PSLICE; pl.p_slices = count; }
+            }
+        }
+    } else {
+        const int wy = nc == 6 ? 2 : 4, ev = 4 * wy;
+        pl.tiles = ((n_omega + 15) / 16) * ((n_thx + 15) / 16) * ((n_thy + 4 * wy - 1) / (4 * wy));
+        pl.t_pad = (int64_t)pl.tiles * SEP_CONS;
+        per_thread_p = ev; per_thread_t = (size_t)nc * ev;
+        // one CTA per SM: the fewest slices k whose tiles*k CTAs fill whole waves to >= 95 %
+        if (pl.tiles < 8 * sms) {
+            const int64_t kmax = std::max<int64_t>(1, (int64_t)count * std::max(1, pl.cpt / 2));
+            int best_k = 1;
+            double best = 0.0;
+            for (int64_t k = 1; k <= std::min<int64_t>(kmax, 4 * sms); ++k) {
+                const int64_t ctas = (int64_t)pl.tiles * k;
+                const double eff = (double)ctas / (double)((ctas + sms - 1) / sms * sms);
+                if (eff > best + 1e-9) { best = eff; best_k = (int)k; }
+                if (eff >= 0.95) break;
+            }
+            if (best_k > 1) {
+                if (count >= best_k) { pl.mode = MODE_PSLICE; pl.p_slices = best_k; }
+                else {
+                    int ts = std::min((best_k + count - 1) / count, std::max(1, pl.cpt / 2));
+                    if (ts > 1) { pl.mode = MODE_TSPLIT; pl.t_slices = ts; pl.p_slices = count; }
+                    else if (count > 1) { pl.mode = MODE_PSLICE; pl.p_slices = count; }
+                }
+            }
         }
     }
     size_t off = 0;
@@ -499,8 +548,8 @@ static Plan make_plan(int count, int64_t n_max, int n_omega, int n_thx, int n_th
     pl.off_n = off;      off += align_up((size_t)count * sizeof(int64_t), 256);
     pl.off_lam = off;    off += align_up((size_t)count * sizeof(double), 256);
     pl.off_partial = off;
-    if (pl.mode == MODE_PSLICE) off += align_up((size_t)pl.p_slices * W * pl.t_pad * 8, 256);
-    if (pl.mode == MODE_TSPLIT) off += align_up((size_t)count * pl.t_slices * nc * W * pl.t_pad * 8, 256);
+    if (pl.mode == MODE_PSLICE) off += align_up((size_t)pl.p_slices * per_thread_p * pl.t_pad * 8, 256);
+    if (pl.mode == MODE_TSPLIT) off += align_up((size_t)count * pl.t_slices * per_thread_t * pl.t_pad * 8, 256);
     pl.total = off;
     return pl;
 }
@@ -524,6 +573,20 @@ static cudaError_t launch_main(const MainParams &mp, dim3 grid, cudaStream_t st)
     return cudaGetLastError();
 }
 
+template <int NC, int WY>
+static cudaError_t launch_sep(const MainParams &mp, dim3 grid, cudaStream_t st) {
+    static std::once_flag once;
+    static cudaError_t attr_err = cudaSuccess;
+    std::call_once(once, [] {
+        attr_err = cudaFuncSetAttribute(rad_sep_kernel<NC, WY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
+                                        SepShape<NC, WY>::SMEM);
+    });
+    if (attr_err != cudaSuccess) return attr_err;
+    rad_sep_kernel<NC, WY><<<grid, SEP_T, SepShape<NC, WY>::SMEM, st>>>(mp);
+    ++g_launches;
+    return cudaGetLastError();
+}
+
 // Everything: pack, main, finalize.  All device pointers; n_host / lam_host are host arrays.
 static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const rad_grid *g, int model,
                      const double *lam_host, int accumulate, double *out,
@@ -542,7 +605,8 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const rad_g
         if (model != RAD_CLASSICAL && !(lam_host[p] >= 0.0)) return RAD_EDOMAIN;
     }
     const int nc = model == RAD_SPIN_HALF ? 6 : 4;
-    const Plan pl = make_plan(b->count, n_max, g->n_omega, g->n_thx, g->n_thy, nc);
+    const Plan pl = make_plan(b->count, n_max, g->n_omega, g->n_thx, g->n_thy, nc,
+                              choose_kernel(g->n_omega, g->n_thx, g->n_thy, nc));
     if (workspace && (reinterpret_cast<uintptr_t>(workspace) & 255)) return RAD_EINVAL;
     if (workspace && workspace_bytes < pl.total) return RAD_ENOSPACE;
     bool own = false;
@@ -585,12 +649,19 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const rad_g
     mp.t_pad = pl.t_pad;
     const int slices = pl.mode == MODE_TSPLIT ? b->count * pl.t_slices : pl.p_slices;
     dim3 grid((unsigned)pl.tiles, (unsigned)slices);
-    cudaError_t e = nc == 6 ? launch_main<6, RAD_DEG>(mp, grid, st) : launch_main<4, RAD_DEG>(mp, grid, st);
-    if (e != cudaSuccess) return cuda_fail(e, "rad_main_kernel");
+    cudaError_t e;
+    if (pl.kernel == 1) e = nc == 6 ? launch_sep<6, 2>(mp, grid, st) : launch_sep<4, 4>(mp, grid, st);
+    else e = nc == 6 ? launch_main<6, RAD_DEG>(mp, grid, st) : launch_main<4, RAD_DEG>(mp, grid, st);
+    if (e != cudaSuccess) return cuda_fail(e, pl.kernel == 1 ? "rad_sep_kernel" : "rad_main_kernel");
     prof_mark(2, st);
     if (pl.mode != MODE_DIRECT) {
-        if (nc == 6) rad_finalize_kernel<6><<<pl.tiles, TPB, 0, st>>>(mp);
-        else rad_finalize_kernel<4><<<pl.tiles, TPB, 0, st>>>(mp);
+        if (pl.kernel == 1) {
+            if (nc == 6) rad_sep_finalize_kernel<6, 2><<<pl.tiles, SEP_CONS, 0, st>>>(mp);
+            else rad_sep_finalize_kernel<4, 4><<<pl.tiles, SEP_CONS, 0, st>>>(mp);
+        } else {
+            if (nc == 6) rad_finalize_kernel<6><<<pl.tiles, TPB, 0, st>>>(mp);
+            else rad_finalize_kernel<4><<<pl.tiles, TPB, 0, st>>>(mp);
+        }
         ++g_launches;
         CK(cudaGetLastError());
         prof_mark(3, st);
@@ -661,7 +732,11 @@ int rad_sum_cubes(const double *cubes, int32_t count, int64_t m, int accumulate,
 
 size_t rad_workspace_bytes(int32_t count, int64_t n_max, int32_t n_omega, int32_t n_thx, int32_t n_thy) {
     if (count < 1 || n_max < 2 || n_omega < 1 || n_thx < 1 || n_thy < 1) return 0;
-    return make_plan(count, n_max, n_omega, n_thx, n_thy, 6).total;
+    size_t need = 0;                                   // whichever kernel and variant the call ends up using
+    for (int kernel = 0; kernel < 2; ++kernel)
+        for (int nc = 4; nc <= 6; nc += 2)
+            need = std::max(need, make_plan(count, n_max, n_omega, n_thx, n_thy, nc, kernel).total);
+    return need;
 }
 
 // ---- host-buffer variants: H2D once, compute, D2H once
@@ -743,6 +818,12 @@ double rad_measure_fp64_peak(double millis, void *cuda_stream) {
 }
 
 int64_t rad_launch_count(void) { return g_launches.load(); }
+
+int rad_set_kernel(int choice) {
+    if (choice < 0 || choice > 2) return RAD_EINVAL;
+    g_kernel_choice.store(choice);
+    return RAD_OK;
+}
 
 int rad_profile_enable(int on) {
     g_prof.store(on ? 1 : 0);

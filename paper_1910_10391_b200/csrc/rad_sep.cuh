@@ -1,0 +1,489 @@
+// rad_sep.cuh -- separable-phasor kernel for tensor angle grids.
+//
+// Eq. (7) on a tensor grid separates exactly, because theta^2 = n_x^2 + n_y^2:
+//     omega* psi = omega* [ (t/2gamma^2 - dz) + (n_x^2 t/2 - n_x x) ]  +  omega* [ n_y^2 t/2 - n_y y ]
+//     e^{i omega* psi} = T(omega, n_x, k) * Y(omega, n_y, k)
+// so a CTA that owns a tile of 16 omega x 16 n_x x (4 WY) n_y points needs, per sample, only
+// 256 + 64 WY phasors (one sincos each, exact chunk-relative phase as in rad_main_kernel) instead
+// of 1024 WY, plus the 64 WY omega-independent integrands f_x, f_y (h) of eqs. (3), (4), (12).
+// Per eval what remains is one complex multiply and the complex accumulation (8 or 10 FP64
+// instructions instead of 24 or 26).
+//
+// CTA = 384 threads, warp-specialised (one CTA per SM):
+//   warps 8-11  PRODUCERS (phase A): wait for trajectory chunks (TMA ring), build the T, Y, F (H)
+//               tables of SEP_S samples per sub-block into a ring of SEP_NB table buffers in
+//               shared memory (structure of arrays: one 8-byte plane per component).
+//   warps 0-7   CONSUMERS (phase B): thread tile 2 omega x 2 n_x x WY n_y (WY = 4 with 4
+//               accumulators per point, WY = 2 with 6); per sample 20 table entries are read
+//               and 16 (8) points updated.  Lane = (l_w, l_x, l_y) = (1, 2, 2) bits, warp =
+//               (w_w, w_x) = (2, 1) bits; the table layouts put the entries one load touches
+//               across a warp into one contiguous piece of shared memory (8 or 16 distinct words).
+// full[] / empty[] mbarriers hand table buffers over; setmaxnreg moves registers from the
+// producers (104) to the consumers (200), whose accumulators need them.
+#pragma once
+
+namespace rad {
+
+constexpr int SEP_CONS = 256;  // consumer threads
+constexpr int SEP_PROD = 128;  // producer threads
+constexpr int SEP_T = SEP_CONS + SEP_PROD;
+constexpr int SEP_S = 4;       // samples per table sub-block
+constexpr int SEP_NB = 3;      // table buffers in flight
+constexpr int SEP_STAGES = 3;  // trajectory-chunk ring depth
+constexpr int SEP_REGS_LAUNCH = 168;                         // __launch_bounds__(384, 1): 65536 / 384 rounded down to 8
+constexpr int SEP_REGS_CONS = 200, SEP_REGS_PROD = 104;          // 256 * 200 + 128 * 104 = 384 * 168: the pool the CTA got at launch
+static_assert(SEP_CONS * SEP_REGS_CONS + SEP_PROD * SEP_REGS_PROD <= SEP_T * SEP_REGS_LAUNCH,
+              "setmaxnreg.inc would wait forever for registers the CTA does not own");
+
+template <int NC, int WY>
+struct SepShape {
+    static constexpr int YN = 64 * WY;            // entries of the Y and F tables per sample
+    static constexpr int EV = 4 * WY;             // grid points per consumer thread
+    static constexpr int PLANE_T = SEP_NB * SEP_S * 256 * 8;     // bytes of one T plane (re or im)
+    static constexpr int PLANE_Y = SEP_NB * SEP_S * YN * 8;      // bytes of one Y / F / H plane
+    static constexpr int OFF_T = SEP_STAGES * CHUNK_BYTES;       // Tre, Tim
+    static constexpr int OFF_Y = OFF_T + 2 * PLANE_T;            // Yre, Yim
+    static constexpr int OFF_F = OFF_Y + 2 * PLANE_Y;            // Fx, Fy
+    static constexpr int OFF_H = OFF_F + 2 * PLANE_Y;            // H (spin-1/2 only)
+    static constexpr int OFF_BAR = OFF_H + (NC == 6 ? PLANE_Y : 0);
+    static constexpr int SMEM = OFF_BAR + (SEP_STAGES + 2 * SEP_NB) * 8;
+};
+
+// Grid coordinates of a thread's EV points.  blockIdx.x enumerates (omega tile, y tile, x tile),
+// x fastest.  Point e = (i * 2 + j) * WY + m  <->  omega index iw0 + i, x index ix0 + j, y index iy0 + m.
+template <int WY>
+struct SepCoord {
+    int bw, bx, by;                  // first omega / x / y index of the CTA tile
+    int iw0, ix0, iy0;               // first omega / x / y index of this thread's points
+    int lw, lx, ly, ww, wx;
+    __device__ __forceinline__ SepCoord(int block, int tid, int n_thx, int n_thy) {
+        const int ntx = (n_thx + 15) / 16, nty = (n_thy + 4 * WY - 1) / (4 * WY);
+        bx = (block % ntx) * 16;
+        by = ((block / ntx) % nty) * 4 * WY;
+        bw = (block / (ntx * nty)) * 16;
+        const int lane = tid & 31, warp = tid >> 5;
+        lw = lane >> 4; lx = (lane >> 2) & 3; ly = lane & 3;
+        ww = warp >> 1; wx = warp & 1;
+        iw0 = bw + 4 * ww + 2 * lw;
+        ix0 = bx + 8 * wx + 2 * lx;
+        iy0 = by + WY * ly;
+    }
+};
+
+// omega* / 2 pi as a double-double, shared by both kernels' prologues
+__device__ __forceinline__ dd omega_star_turns(double om, double lam) {
+    dd u = two_prod(om, lam);
+    dd d = two_sum(1.0, -u.hi);
+    d = fast_two_sum(d.hi, d.lo - u.lo);          // 1 - u
+    dd wst = d_div_dd(om, d);                     // omega / (1 - u)
+    return dd_mul(wst, dd{INV_2PI_HI, INV_2PI_LO});
+}
+
+__device__ __forceinline__ dd half_square_dd(double a) {      // a^2 / 2
+    dd s = two_prod(a, a);
+    return {0.5 * s.hi, 0.5 * s.lo};
+}
+
+// true (cos, sin) of 2 pi p, high-accuracy polynomial set (tables are built once per 16 evals)
+__device__ __forceinline__ double2 phasor_full(double p) {
+    double c, s;
+    phasor_turns<6>(p, c, s);
+    return make_double2(c, s * 1.4142135623730951);
+}
+
+// spectrum value from true complex amplitudes acc = (Re Ax, Im Ax, Re Ay, Im Ay[, Re J, Im J])
+template <int NC>
+__device__ __forceinline__ double spectrum_value_true(const double *acc, double nx, double ny,
+                                                      int model, double u, double gamma0) {
+    const double INV_4PI2 = 0.025330295910584442860969;
+    const double azr = -(nx * acc[0] + ny * acc[2]);
+    const double azi = -(nx * acc[1] + ny * acc[3]);
+    const double S = acc[0] * acc[0] + acc[1] * acc[1] + acc[2] * acc[2] + acc[3] * acc[3]
+                   + azr * azr + azi * azi;
+    if (!(u < 1.0)) return __longlong_as_double(0x7ff8000000000000LL);
+    if (model == RAD_CLASSICAL) return S * INV_4PI2;
+    const double e = 1.0 - u;
+    if (model == RAD_SPIN0) return e * S * INV_4PI2;
+    double J2 = 0.0;
+    if (NC == 6) J2 = acc[4] * acc[4] + acc[5] * acc[5];
+    return (0.5 * (1.0 + e * e) * S + u * u / (2.0 * gamma0 * gamma0) * J2) * INV_4PI2;
+}
+
+// ------------------------------------------------------------------------------ small PTX helpers
+__device__ __forceinline__ void mbar_arrive(uint64_t *bar) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];" ::"r"(smem_u32(bar)) : "memory");
+}
+template <int REGS> __device__ __forceinline__ void reg_alloc() {
+    asm volatile("setmaxnreg.inc.sync.aligned.u32 %0;" ::"n"(REGS));
+}
+template <int REGS> __device__ __forceinline__ void reg_dealloc() {
+    asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REGS));
+}
+__device__ __forceinline__ void producer_bar_sync() {          // named barrier 1: the 128 producer threads
+    asm volatile("bar.sync 1, 128;" ::: "memory");
+}
+
+// The sequence of (trajectory, chunk, sub-block) steps of one CTA.  Producers and consumers each run
+// their own copy: both sides derive the same sequence from the launch parameters, so the only thing
+// they exchange is table buffers.
+struct SepCursor {
+    int p, p_end, ts;
+    int c, c1;                 // chunk index, end of this trajectory's chunk range
+    int sb, nsb;               // sub-block inside the chunk, sub-blocks of this chunk
+    __device__ __forceinline__ SepCursor(const MainParams &P, int slice) {
+        ts = 0;
+        if (P.mode == MODE_TSPLIT) { p = slice / P.t_slices; p_end = p + 1; ts = slice % P.t_slices; }
+        else { p = (int)((int64_t)slice * P.count / P.p_slices);
+               p_end = (int)((int64_t)(slice + 1) * P.count / P.p_slices); }
+        sb = 0; nsb = 0; c = 0; c1 = 0;
+        seek(P);
+    }
+    static __device__ __forceinline__ int64_t n_of(const MainParams &P, int q) {
+        return P.n_dev ? P.n_dev[q] : P.n_single;
+    }
+    __device__ __forceinline__ void chunk_range(const MainParams &P, int q, int &c0, int &cend) const {
+        const int nch = (int)((n_of(P, q) + CH - 1) / CH);
+        if (P.mode == MODE_TSPLIT) { c0 = (int)((int64_t)ts * nch / P.t_slices);
+                                     cend = (int)((int64_t)(ts + 1) * nch / P.t_slices); }
+        else { c0 = 0; cend = nch; }
+    }
+    __device__ __forceinline__ void set_nsb(const MainParams &P) {
+        const int64_t left = n_of(P, p) - (int64_t)c * CH;
+        nsb = ((int)min((int64_t)CH, left) + SEP_S - 1) / SEP_S;
+    }
+    __device__ __forceinline__ void seek(const MainParams &P) {   // first trajectory from p on with chunks to do
+        while (p < p_end) {
+            chunk_range(P, p, c, c1);
+            if (c < c1) { set_nsb(P); break; }
+            ++p;
+        }
+    }
+    __device__ __forceinline__ bool valid() const { return p < p_end; }
+    // advance by one sub-block; returns 0 (same chunk), 1 (chunk finished), 2 (trajectory finished)
+    __device__ __forceinline__ int step(const MainParams &P) {
+        if (++sb < nsb) return 0;
+        sb = 0;
+        if (++c < c1) { set_nsb(P); return 1; }
+        ++p;
+        seek(P);
+        return 2;
+    }
+};
+
+// ------------------------------------------------------------------------------ main (a0-a7)
+template <int NC, int WY>
+__global__ void __launch_bounds__(SEP_T, 1)
+rad_sep_kernel(const MainParams P) {
+    using SH = SepShape<NC, WY>;
+    constexpr int YN = SH::YN, EV = SH::EV, S = SEP_S, NB = SEP_NB;
+    extern __shared__ __align__(128) unsigned char smem_raw[];
+    double *ring = reinterpret_cast<double *>(smem_raw);
+    double *Tre = reinterpret_cast<double *>(smem_raw + SH::OFF_T);       // [NB][S][256]
+    double *Tim = Tre + NB * S * 256;
+    double *Yre = reinterpret_cast<double *>(smem_raw + SH::OFF_Y);       // [NB][S][YN]
+    double *Yim = Yre + NB * S * YN;
+    double *Fx = reinterpret_cast<double *>(smem_raw + SH::OFF_F);        // [NB][S][YN]  w f_x, w f_y
+    double *Fy = Fx + NB * S * YN;
+    double *Hh = reinterpret_cast<double *>(smem_raw + SH::OFF_H);        // [NB][S][YN]  w h (spin-1/2)
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem_raw + SH::OFF_BAR);   // trajectory stages
+    uint64_t *full = bars + SEP_STAGES, *empty = full + NB;
+    const int tid = threadIdx.x;
+    const int slice = blockIdx.y;
+
+    if (tid == 0) {
+        for (int s = 0; s < SEP_STAGES; ++s) mbar_init(&bars[s], 1);
+        for (int b = 0; b < NB; ++b) { mbar_init(&full[b], SEP_PROD / 32); mbar_init(&empty[b], SEP_CONS / 32); }
+        mbar_fence_init();
+    }
+    __syncthreads();
+
+    if (tid >= SEP_CONS) {
+        // ====================================================================== PRODUCERS (phase A)
+        reg_dealloc<SEP_REGS_PROD>();
+        const int pt = tid - SEP_CONS;
+        const int tile_bx = blockIdx.x;
+        const SepCoord<WY> co(tile_bx, 0, P.n_thx, P.n_thy);             // tile bases only
+        constexpr int RT = 256 / SEP_PROD, RY = YN / SEP_PROD;           // entries per thread and table
+        double omT[RT], nxT[RT], omY[RY], nyY[RY], nxF[RY], nyF[RY], hF[RY];
+#pragma unroll
+        for (int r = 0; r < RT; ++r) {
+            const int b = pt + r * SEP_PROD;
+            const int iw = co.bw + 4 * (b >> 6) + 2 * ((b >> 2) & 1) + ((b >> 4) & 1);
+            const int ix = co.bx + 8 * ((b >> 5) & 1) + 2 * (b & 3) + ((b >> 3) & 1);
+            omT[r] = P.omega[min(iw, P.n_omega - 1)];
+            nxT[r] = P.thx[min(ix, P.n_thx - 1)];
+        }
+#pragma unroll
+        for (int r = 0; r < RY; ++r) {
+            const int b = pt + r * SEP_PROD;
+            {
+                const int q = b >> 3, m = q % WY, i = (q / WY) & 1, ww = (q / WY) >> 1;
+                const int iw = co.bw + 4 * ww + 2 * ((b >> 2) & 1) + i;
+                const int iy = co.by + WY * (b & 3) + m;
+                omY[r] = P.omega[min(iw, P.n_omega - 1)];
+                nyY[r] = P.thy[min(iy, P.n_thy - 1)];
+            }
+            {
+                const int q = b >> 4, m = q % WY, j = (q / WY) & 1, wx = (q / WY) >> 1;
+                const int ix = co.bx + 8 * wx + 2 * ((b >> 2) & 3) + j;
+                const int iy = co.by + WY * (b & 3) + m;
+                nxF[r] = P.thx[min(ix, P.n_thx - 1)];
+                nyF[r] = P.thy[min(iy, P.n_thy - 1)];
+                hF[r] = 0.5 * (nxF[r] * nxF[r] + nyF[r] * nyF[r]);
+            }
+        }
+
+        // TMA producer cursor (thread pt == 0 only): its own copy of the step sequence, chunk by chunk
+        SepCursor tc(P, slice);
+        uint32_t issued = 0;
+        auto produce = [&]() {
+            if (!tc.valid()) return;
+            const int s = issued % SEP_STAGES;
+            mbar_expect_tx(&bars[s], CHUNK_BYTES);
+            tma_load_1d(ring + (size_t)s * CHUNK_DBL,
+                        P.packed + ((int64_t)tc.p * P.cpt + tc.c) * CHUNK_DBL, CHUNK_BYTES, &bars[s]);
+            ++issued;
+            tc.sb = tc.nsb - 1;                          // jump to the end of the chunk
+            tc.step(P);
+        };
+        if (pt == 0)
+            for (int s = 0; s < SEP_STAGES; ++s) produce();
+
+        SepCursor cur(P, slice);
+        uint32_t it = 0, g = 0;                          // chunks consumed, sub-blocks produced
+        while (cur.valid()) {
+            // ---- new chunk: wait for it, exact base phases of this thread's entries (a3)
+            const int st = it % SEP_STAGES;
+            mbar_wait(&bars[st], (it / SEP_STAGES) & 1);
+            const double *ck = ring + (size_t)st * CHUNK_DBL;
+            const double lam = P.lam_dev ? P.lam_dev[cur.p] : P.lam_single;
+            double p0T[RT], whT[RT], hxT[RT], p0Y[RY], whY[RY], hyY[RY];
+            {
+                const double2 h01 = *reinterpret_cast<const double2 *>(ck);        // P0_b hi, lo
+                const double2 h23 = *reinterpret_cast<const double2 *>(ck + 2);    // t_b, x_b
+                const double yb = ck[4];
+#pragma unroll
+                for (int r = 0; r < RT; ++r) {
+                    const dd wt = omega_star_turns(omT[r], lam);
+                    const dd hx = half_square_dd(nxT[r]);
+                    dd psi = {h01.x, h01.y};
+                    psi = dd_add(psi, dd_mul_d(hx, h23.x));
+                    psi = dd_add(psi, dd_neg(two_prod(nxT[r], h23.y)));
+                    p0T[r] = dd_frac(dd_mul(wt, psi));
+                    whT[r] = wt.hi; hxT[r] = hx.hi;
+                }
+#pragma unroll
+                for (int r = 0; r < RY; ++r) {
+                    const dd wt = omega_star_turns(omY[r], lam);
+                    const dd hy = half_square_dd(nyY[r]);
+                    dd psi = dd_mul_d(hy, h23.x);
+                    psi = dd_add(psi, dd_neg(two_prod(nyY[r], yb)));
+                    p0Y[r] = dd_frac(dd_mul(wt, psi));
+                    whY[r] = wt.hi; hyY[r] = hy.hi;
+                }
+            }
+            int adv = 0;
+            do {                                         // sub-blocks of this chunk
+                const int buf = g % NB;
+                mbar_wait(&empty[buf], ((g / NB) & 1) ^ 1);
+                const double *rec = ck + HDR + cur.sb * S * REC;
+#pragma unroll 1
+                for (int s = 0; s < S; ++s, rec += REC) {
+                    const int row = buf * S + s;
+                    const double2 r67 = *reinterpret_cast<const double2 *>(rec + 6);   // dP0, dt
+                    const double2 r89 = *reinterpret_cast<const double2 *>(rec + 8);   // dx, dy
+#pragma unroll
+                    for (int r = 0; r < RT; ++r) {
+                        const double dT = fma(-nxT[r], r89.x, fma(hxT[r], r67.y, r67.x));
+                        const double2 ph = phasor_full(fma(whT[r], dT, p0T[r]));
+                        Tre[row * 256 + pt + r * SEP_PROD] = ph.x;
+                        Tim[row * 256 + pt + r * SEP_PROD] = ph.y;
+                    }
+#pragma unroll
+                    for (int r = 0; r < RY; ++r) {
+                        const double dY = fma(-nyY[r], r89.y, hyY[r] * r67.y);
+                        const double2 ph = phasor_full(fma(whY[r], dY, p0Y[r]));
+                        Yre[row * YN + pt + r * SEP_PROD] = ph.x;
+                        Yim[row * YN + pt + r * SEP_PROD] = ph.y;
+                    }
+                    const double2 r01 = *reinterpret_cast<const double2 *>(rec);       // D0, vx
+                    const double2 r23 = *reinterpret_cast<const double2 *>(rec + 2);   // vy, w ax
+                    const double2 r45 = *reinterpret_cast<const double2 *>(rec + 4);   // w ay, w az
+#pragma unroll
+                    for (int r = 0; r < RY; ++r) {       // a2: eqs. (3), (4), (6), (12), times the weight
+                        const double D = r01.x - hF[r];
+                        const double ux = nxF[r] - r01.y, uy = nyF[r] - r23.x;
+                        const double bx = fma(nyF[r], uy, D);
+                        const double by = fma(nxF[r], ux, D);
+                        const double q = fma(nxF[r], ux, bx);
+                        const double gq = inv_square(q);
+                        const double s1 = fma(nyF[r], r45.x, r45.y);
+                        const double s2 = fma(nxF[r], r23.y, r45.y);
+                        Fx[row * YN + pt + r * SEP_PROD] = fma(s1, ux, -(bx * r23.y)) * gq;
+                        Fy[row * YN + pt + r * SEP_PROD] = fma(s2, uy, -(by * r45.x)) * gq;
+                        if (NC == 6) Hh[row * YN + pt + r * SEP_PROD] = fma(nxF[r], r23.y, s1) * gq;
+                    }
+                }
+                __syncwarp();
+                if ((pt & 31) == 0) mbar_arrive(&full[buf]);
+                ++g;
+                adv = cur.step(P);
+            } while (adv == 0);
+            // ---- chunk finished by every producer: its ring stage can be refilled
+            ++it;
+            producer_bar_sync();
+            if (pt == 0) produce();
+        }
+        return;
+    }
+
+    // ========================================================================== CONSUMERS (phase B)
+    reg_alloc<SEP_REGS_CONS>();
+    const SepCoord<WY> co(blockIdx.x, tid, P.n_thx, P.n_thy);
+    const int64_t gid = (int64_t)blockIdx.x * SEP_CONS + tid;
+    // read offsets (entries) of this thread inside one sample's tables
+    const int rT = (co.ww * 2 + co.wx) * 32 + co.lw * 4 + co.lx;          // + (i*2 + j) * 8
+    const int rY = co.ww * 2 * WY * 8 + co.lw * 4 + co.ly;                // + (i*WY + m) * 8
+    const int rF = co.wx * 2 * WY * 16 + co.lx * 4 + co.ly;               // + (j*WY + m) * 16
+
+    // ---- output slots of this thread: zero them, later every trajectory adds its spectrum
+    const int A = P.n_thx * P.n_thy;
+    auto out_slot = [&](int e) -> double * {          // nullptr: point outside the grid
+        const int m = e % WY, j = (e / WY) & 1, i = e / (2 * WY);
+        const int iw = co.iw0 + i, ix = co.ix0 + j, iy = co.iy0 + m;
+        if (P.mode == MODE_PSLICE) return P.partial + ((int64_t)slice * EV + e) * P.t_pad + gid;
+        if (iw >= P.n_omega || ix >= P.n_thx || iy >= P.n_thy) return nullptr;
+        return P.out + (int64_t)iw * A + (int64_t)iy * P.n_thx + ix;
+    };
+    if (P.mode != MODE_TSPLIT && !(P.mode == MODE_DIRECT && P.accumulate)) {
+#pragma unroll 1
+        for (int e = 0; e < EV; ++e) {
+            double *o = out_slot(e);
+            if (o) *o = 0.0;
+        }
+    }
+
+    double acc[EV][NC];
+#pragma unroll
+    for (int e = 0; e < EV; ++e)
+#pragma unroll
+        for (int c = 0; c < NC; ++c) acc[e][c] = 0.0;
+
+    SepCursor cur(P, slice);
+    if (P.mode == MODE_TSPLIT && !cur.valid()) {      // empty time slice: its partial amplitudes are zero
+        double *dst = P.partial + (int64_t)slice * NC * EV * P.t_pad + gid;
+        for (int k = 0; k < NC * EV; ++k) dst[(int64_t)k * P.t_pad] = 0.0;
+    }
+    uint32_t g = 0;
+    while (cur.valid()) {
+        const int p_now = cur.p;
+        const int buf = g % NB;
+        mbar_wait(&full[buf], (g / NB) & 1);
+#pragma unroll 1
+        for (int s = 0; s < S; ++s) {                 // a4: complex multiply + accumulate
+            const int row = buf * S + s;
+            const double *tre = Tre + row * 256 + rT, *tim = Tim + row * 256 + rT;
+            const double *yre = Yre + row * YN + rY, *yim = Yim + row * YN + rY;
+            const double *fxp = Fx + row * YN + rF, *fyp = Fy + row * YN + rF, *hp = Hh + row * YN + rF;
+            double tr[2][2], ti[2][2];
+#pragma unroll
+            for (int i = 0; i < 2; ++i)
+#pragma unroll
+                for (int j = 0; j < 2; ++j) { tr[i][j] = tre[(i * 2 + j) * 8]; ti[i][j] = tim[(i * 2 + j) * 8]; }
+#pragma unroll
+            for (int m = 0; m < WY; ++m) {
+                double yr[2], yi[2];
+#pragma unroll
+                for (int i = 0; i < 2; ++i) { yr[i] = yre[(i * WY + m) * 8]; yi[i] = yim[(i * WY + m) * 8]; }
+#pragma unroll
+                for (int j = 0; j < 2; ++j) {
+                    const double fxv = fxp[(j * WY + m) * 16], fyv = fyp[(j * WY + m) * 16];
+                    double hv = 0.0;
+                    if (NC == 6) hv = hp[(j * WY + m) * 16];
+#pragma unroll
+                    for (int i = 0; i < 2; ++i) {
+                        const double qr = fma(-ti[i][j], yi[i], tr[i][j] * yr[i]);
+                        const double qi = fma(ti[i][j], yr[i], tr[i][j] * yi[i]);
+                        double *a = acc[(i * 2 + j) * WY + m];
+                        a[0] = fma(fxv, qr, a[0]);
+                        a[1] = fma(fxv, qi, a[1]);
+                        a[2] = fma(fyv, qr, a[2]);
+                        a[3] = fma(fyv, qi, a[3]);
+                        if (NC == 6) {
+                            a[4] = fma(hv, qr, a[4]);
+                            a[5] = fma(hv, qi, a[5]);
+                        }
+                    }
+                }
+            }
+        }
+        __syncwarp();
+        if ((tid & 31) == 0) mbar_arrive(&empty[buf]);
+        ++g;
+        if (cur.step(P) == 2) {
+            // ================================================================ end of trajectory p_now (a5, a7)
+            if (P.mode == MODE_TSPLIT) {
+                double *dst = P.partial + (int64_t)slice * NC * EV * P.t_pad + gid;
+#pragma unroll
+                for (int e = 0; e < EV; ++e)
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) dst[(int64_t)(c * EV + e) * P.t_pad] = acc[e][c];
+            } else {
+                const double lam = P.lam_dev ? P.lam_dev[p_now] : P.lam_single;
+                const double gamma0 = P.packed[(int64_t)p_now * P.cpt * CHUNK_DBL + 5];
+#pragma unroll
+                for (int e = 0; e < EV; ++e) {
+                    const int m = e % WY, j = (e / WY) & 1, i = e / (2 * WY);
+                    const double om = P.omega[min(co.iw0 + i, P.n_omega - 1)];
+                    const double nx = P.thx[min(co.ix0 + j, P.n_thx - 1)];
+                    const double ny = P.thy[min(co.iy0 + m, P.n_thy - 1)];
+                    double *o = out_slot(e);
+                    if (o) *o += spectrum_value_true<NC>(acc[e], nx, ny, P.model, om * lam, gamma0);
+                }
+            }
+#pragma unroll
+            for (int e = 0; e < EV; ++e)
+#pragma unroll
+                for (int c = 0; c < NC; ++c) acc[e][c] = 0.0;
+        }
+    }
+}
+
+// ------------------------------------------------------------------------------ finalize (a6, a7)
+template <int NC, int WY>
+__global__ void __launch_bounds__(SEP_CONS)
+rad_sep_finalize_kernel(const MainParams P) {
+    constexpr int EV = 4 * WY;
+    const SepCoord<WY> co(blockIdx.x, threadIdx.x, P.n_thx, P.n_thy);
+    const int64_t gid = (int64_t)blockIdx.x * SEP_CONS + threadIdx.x;
+    const int A = P.n_thx * P.n_thy;
+    for (int e = 0; e < EV; ++e) {
+        const int m = e % WY, j = (e / WY) & 1, i = e / (2 * WY);
+        const int iw = co.iw0 + i, ix = co.ix0 + j, iy = co.iy0 + m;
+        if (iw >= P.n_omega || ix >= P.n_thx || iy >= P.n_thy) continue;
+        double total = 0.0;
+        if (P.mode == MODE_PSLICE) {
+            for (int s = 0; s < P.p_slices; ++s)                       // slices ascending
+                total += P.partial[((int64_t)s * EV + e) * P.t_pad + gid];
+        } else {
+            const double om = P.omega[iw], nx = P.thx[ix], ny = P.thy[iy];
+            for (int p = 0; p < P.count; ++p) {                        // trajectories ascending
+                double acc[NC];
+#pragma unroll
+                for (int c = 0; c < NC; ++c) acc[c] = 0.0;
+                for (int s = 0; s < P.t_slices; ++s) {                 // time slices ascending
+                    const double *src = P.partial + (int64_t)(p * P.t_slices + s) * NC * EV * P.t_pad + gid;
+#pragma unroll
+                    for (int c = 0; c < NC; ++c) acc[c] += src[(int64_t)(c * EV + e) * P.t_pad];
+                }
+                const double lam = P.lam_dev ? P.lam_dev[p] : P.lam_single;
+                const double gamma0 = P.packed[(int64_t)p * P.cpt * CHUNK_DBL + 5];
+                total += spectrum_value_true<NC>(acc, nx, ny, P.model, om * lam, gamma0);
+            }
+        }
+        double *o = P.out + (int64_t)iw * A + (int64_t)iy * P.n_thx + ix;
+        *o = P.accumulate ? *o + total : total;
+    }
+}
+
+}  // namespace rad

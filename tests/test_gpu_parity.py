@@ -330,3 +330,90 @@ def test_shards_run_sequentially_equal_unsharded(rad, oracle_mod):
     total = rad.rad_sum_cubes(torch.stack(parts)).cpu().numpy()
     w, nx, ny = oracle_mod.grid_points(we.omega, we.thx, we.thy)
     assert_parity(total, oracle_mod.ensemble_points(we.batch, we.n, w, nx, ny), label="ensemble shards")
+
+
+# ------------------------------------------------------------------ separable-phasor kernel (N2), forced
+@pytest.fixture
+def sep_kernel(rad):
+    rad.rad_set_kernel(2)
+    yield rad
+    rad.rad_set_kernel(0)
+
+
+@pytest.mark.parametrize("model", [CL, S0, SH])
+@pytest.mark.parametrize("shape", [dict(n=2, n_omega=1, n_th=1), dict(n=131, n_omega=17, n_th=5),
+                                   dict(n=1037, n_omega=33, n_th=19)])
+def test_sep_ragged_shapes_all_models(sep_kernel, oracle_mod, model, shape):
+    """Separable kernel on grids that are not multiples of its 16 x 16 x 16 (8) tiles, n not a multiple
+    of the 4-sample sub-block or the 128-sample chunk (time-split plan)."""
+    wl = workloads.make("cfg2", seed=12, **shape)
+    lam = 0.6 / wl.omega.max()
+    cube = run_single(sep_kernel, wl, model, lam)
+    ref = oracle_mod.grid(wl.traj, wl.omega, wl.thx, wl.thy, model, lam)
+    assert_parity(cube, ref, label=f"sep ragged {shape} model {model}")
+
+
+def test_sep_rectangular_and_nonuniform(sep_kernel, oracle_mod):
+    wl = workloads.make("cfg2", n=900, n_omega=10, n_th=21, seed=8)
+    wl.thx = wl.thx[:18].copy()
+    wl.thy = (wl.thy[:9] * 0.7).copy()
+    rng = np.random.Generator(np.random.PCG64(3))
+    t = np.sort(rng.uniform(0, wl.traj["t"][-1], 900))
+    tr = {k: np.interp(t, wl.traj["t"], v) for k, v in wl.traj.items()}
+    tr["t"] = t
+    tr["gamma"] = wl.traj["gamma"] * (1 - 1e-3 * np.linspace(0, 1, 900))
+    wl.traj = tr
+    lam = 0.5 / wl.omega.max()
+    for model in (CL, SH):
+        cube = run_single(sep_kernel, wl, model, lam)
+        assert cube.shape == (10, 9, 18)
+        ref = oracle_mod.grid(tr, wl.omega, wl.thx, wl.thy, model, lam)
+        assert_parity(cube, ref, label=f"sep rectangular nonuniform model {model}")
+
+
+def test_sep_direct_mode_and_determinism(sep_kernel, oracle_mod):
+    """Enough tiles for the no-split plan (>= 8 per SM); two runs give the same bits."""
+    wl = workloads.make("cfg2", n=300, n_omega=80, n_th=256, seed=21)
+    cube = run_single(sep_kernel, wl, CL, 0.0)
+    idx, ref = sampled_reference(oracle_mod, wl, cube, 3000, (5, 9, 9), CL, 0.0)
+    assert_parity(cube, ref, idx, label="sep direct")
+    assert np.array_equal(cube, run_single(sep_kernel, wl, CL, 0.0))
+
+
+@pytest.mark.parametrize("model", [CL, SH])
+def test_sep_ensembles(sep_kernel, oracle_mod, model):
+    """Few ragged trajectories (time split) and many short ones (trajectory split) + accumulate."""
+    we = workloads.make("cfg4", count=6, n=700, n_omega=9, n_th=5)
+    nvec = np.array([700, 512, 129, 2, 700, 333], dtype=np.int64)
+    lam = np.linspace(0.2, 0.7, 6) / we.omega.max() if model != CL else None
+    cube = sep_kernel.rad_ensemble_sum(dev_dict(we.batch), nvec, *dev_grid(we), model=model,
+                                       hbarc_over_E=lam).cpu().numpy()
+    w, nx, ny = oracle_mod.grid_points(we.omega, we.thx, we.thy)
+    assert_parity(cube, oracle_mod.ensemble_points(we.batch, nvec, w, nx, ny, model, lam),
+                  label=f"sep ensemble small model {model}")
+    we = workloads.make("cfg4", count=400, n=300, n_omega=8, n_th=4, seed0=900)
+    rng = np.random.Generator(np.random.PCG64(1))
+    nvec = rng.integers(2, 301, size=400).astype(np.int64)
+    lam = np.full(400, 0.4 / we.omega.max()) if model != CL else None
+    b, g = dev_dict(we.batch), dev_grid(we)
+    ref = oracle_mod.ensemble_points(we.batch, nvec, *oracle_mod.grid_points(we.omega, we.thx, we.thy), model, lam)
+    full = sep_kernel.rad_ensemble_sum(b, nvec, *g, model=model, hbarc_over_E=lam).cpu().numpy()
+    assert_parity(full, ref, label=f"sep ensemble many model {model}")
+    first = sep_kernel.rad_ensemble_sum({k: v[:150].contiguous() for k, v in b.items()}, nvec[:150], *g,
+                                        model=model, hbarc_over_E=None if lam is None else lam[:150])
+    both = sep_kernel.rad_ensemble_sum({k: v[150:].contiguous() for k, v in b.items()}, nvec[150:], *g,
+                                       model=model, hbarc_over_E=None if lam is None else lam[150:],
+                                       accumulate=True, out=first).cpu().numpy()
+    assert_parity(both, ref, label=f"sep ensemble accumulate model {model}")
+
+
+def test_sep_matches_direct_kernel(rad, oracle_mod):
+    """Both kernels on the same input agree far inside the tolerance (they share only the packed records)."""
+    wl = workloads.make("cfg3", n=5000, n_omega=32, n_th=32)
+    rad.rad_set_kernel(1)
+    a = run_single(rad, wl, SH, wl.hbarc_over_E)
+    rad.rad_set_kernel(2)
+    b = run_single(rad, wl, SH, wl.hbarc_over_E)
+    rad.rad_set_kernel(0)
+    tol = np.maximum(RTOL * np.abs(a), FLOOR * a.max())
+    assert np.max(np.abs(a - b) / tol) <= 1.0
