@@ -369,17 +369,27 @@ rad_sep_kernel(const MainParams P) {
 #pragma unroll
         for (int c = 0; c < NC; ++c) acc[e][c] = 0.0;
 
+    // The consumers only need to know how many sub-blocks each trajectory of their slice has.
     SepCursor cur(P, slice);
     if (P.mode == MODE_TSPLIT && !cur.valid()) {      // empty time slice: its partial amplitudes are zero
         double *dst = P.partial + (int64_t)slice * NC * EV * P.t_pad + gid;
         for (int k = 0; k < NC * EV; ++k) dst[(int64_t)k * P.t_pad] = 0.0;
     }
+    int p_now = cur.p;
+    const int p_end = cur.p_end;
+    auto sub_blocks_of = [&](int p) -> int {          // sub-blocks of trajectory p inside this slice
+        int c0, c1;
+        cur.chunk_range(P, p, c0, c1);
+        if (c0 >= c1) return 0;
+        const int64_t left = SepCursor::n_of(P, p) - (int64_t)(c1 - 1) * CH;      // samples of the last chunk
+        return (c1 - 1 - c0) * (CH / S) + ((int)min((int64_t)CH, left) + S - 1) / S;
+    };
+    int todo = p_now < p_end ? sub_blocks_of(p_now) : 0;
     uint32_t g = 0;
-    while (cur.valid()) {
-        const int p_now = cur.p;
+    while (p_now < p_end) {
         const int buf = g % NB;
         mbar_wait(&full[buf], (g / NB) & 1);
-#pragma unroll 1
+#pragma unroll
         for (int s = 0; s < S; ++s) {                 // a4: complex multiply + accumulate
             const int row = buf * S + s;
             const double *tre = Tre + row * 256 + rT, *tim = Tim + row * 256 + rT;
@@ -420,7 +430,7 @@ rad_sep_kernel(const MainParams P) {
         __syncwarp();
         if ((tid & 31) == 0) mbar_arrive(&empty[buf]);
         ++g;
-        if (cur.step(P) == 2) {
+        if (--todo == 0) {
             // ================================================================ end of trajectory p_now (a5, a7)
             if (P.mode == MODE_TSPLIT) {
                 double *dst = P.partial + (int64_t)slice * NC * EV * P.t_pad + gid;
@@ -445,6 +455,10 @@ rad_sep_kernel(const MainParams P) {
             for (int e = 0; e < EV; ++e)
 #pragma unroll
                 for (int c = 0; c < NC; ++c) acc[e][c] = 0.0;
+            do {                                      // next trajectory of the slice that has work
+                ++p_now;
+                todo = p_now < p_end ? sub_blocks_of(p_now) : 0;
+            } while (p_now < p_end && todo == 0);
         }
     }
 }
