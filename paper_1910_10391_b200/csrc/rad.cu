@@ -522,7 +522,7 @@ static Plan make_plan(int count, int64_t n_max, int n_omega, int n_thx, int n_th
         pl.tiles = ((n_omega + 15) / 16) * ((n_thx + 15) / 16) * ((n_thy + 4 * wy - 1) / (4 * wy));
         pl.t_pad = (int64_t)pl.tiles * SEP_CONS;
         per_thread_p = ev; per_thread_t = (size_t)nc * ev;
-        // one CTA per SM: the fewest slices k whose tiles*k CTAs fill whole waves to >= 95 %
+        // one CTA per SM: the fewest slices k whose tiles*k CTAs fill whole waves to >= 98.5 %
         if (pl.tiles < 8 * sms) {
             const int64_t kmax = std::max<int64_t>(1, (int64_t)count * std::max(1, pl.cpt / 2));
             int best_k = 1;
@@ -531,7 +531,7 @@ static Plan make_plan(int count, int64_t n_max, int n_omega, int n_thx, int n_th
                 const int64_t ctas = (int64_t)pl.tiles * k;
                 const double eff = (double)ctas / (double)((ctas + sms - 1) / sms * sms);
                 if (eff > best + 1e-9) { best = eff; best_k = (int)k; }
-                if (eff >= 0.95) break;
+                if (eff >= 0.985) break;
             }
             if (best_k > 1) {
                 if (count >= best_k) { pl.mode = MODE_PSLICE; pl.p_slices = best_k; }

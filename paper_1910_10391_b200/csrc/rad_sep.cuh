@@ -12,12 +12,15 @@
 // CTA = 384 threads, warp-specialised (one CTA per SM):
 //   warps 8-11  PRODUCERS (phase A): wait for trajectory chunks (TMA ring), build the T, Y, F (H)
 //               tables of SEP_S samples per sub-block into a ring of SEP_NB table buffers in
-//               shared memory (structure of arrays: one 8-byte plane per component).
+//               shared memory (16-byte entries: (re, im) of T and Y, (w f_x, w f_y) of F).
 //   warps 0-7   CONSUMERS (phase B): thread tile 2 omega x 2 n_x x WY n_y (WY = 4 with 4
 //               accumulators per point, WY = 2 with 6); per sample 20 table entries are read
-//               and 16 (8) points updated.  Lane = (l_w, l_x, l_y) = (1, 2, 2) bits, warp =
-//               (w_w, w_x) = (2, 1) bits; the table layouts put the entries one load touches
-//               across a warp into one contiguous piece of shared memory (8 or 16 distinct words).
+//               and 16 (8) points updated.  Lane bits (high to low) = (l_x, l_y, l_w) = (2, 2, 1),
+//               warp = (w_w, w_x) = (2, 1) bits; the table layouts put the entries one load touches
+//               across a warp into one contiguous piece of shared memory.  Shared-memory cost is
+//               counted in 128-byte wavefronts of REQUESTS: only lanes 2k, 2k+1 reading the same
+//               address are merged (measured), so l_w is the lowest lane bit -- the
+//               F table (8 entries per thread, independent of omega) then costs half.
 // full[] / empty[] mbarriers hand table buffers over; setmaxnreg moves registers from the
 // producers (104) to the consumers (200), whose accumulators need them.
 #pragma once
@@ -39,13 +42,13 @@ template <int NC, int WY>
 struct SepShape {
     static constexpr int YN = 64 * WY;            // entries of the Y and F tables per sample
     static constexpr int EV = 4 * WY;             // grid points per consumer thread
-    static constexpr int PLANE_T = SEP_NB * SEP_S * 256 * 8;     // bytes of one T plane (re or im)
-    static constexpr int PLANE_Y = SEP_NB * SEP_S * YN * 8;      // bytes of one Y / F / H plane
-    static constexpr int OFF_T = SEP_STAGES * CHUNK_BYTES;       // Tre, Tim
-    static constexpr int OFF_Y = OFF_T + 2 * PLANE_T;            // Yre, Yim
-    static constexpr int OFF_F = OFF_Y + 2 * PLANE_Y;            // Fx, Fy
-    static constexpr int OFF_H = OFF_F + 2 * PLANE_Y;            // H (spin-1/2 only)
-    static constexpr int OFF_BAR = OFF_H + (NC == 6 ? PLANE_Y : 0);
+    static constexpr int BYTES_T = SEP_NB * SEP_S * 256 * 16;    // T table ring: (re, im) per entry
+    static constexpr int BYTES_Y = SEP_NB * SEP_S * YN * 16;     // Y ring (re, im); F ring (w f_x, w f_y)
+    static constexpr int OFF_T = SEP_STAGES * CHUNK_BYTES;
+    static constexpr int OFF_Y = OFF_T + BYTES_T;
+    static constexpr int OFF_F = OFF_Y + BYTES_Y;
+    static constexpr int OFF_H = OFF_F + BYTES_Y;                // H ring: w h, 8 bytes per entry (spin-1/2 only)
+    static constexpr int OFF_BAR = OFF_H + (NC == 6 ? BYTES_Y / 2 : 0);
     static constexpr int SMEM = OFF_BAR + (SEP_STAGES + 2 * SEP_NB) * 8;
 };
 
@@ -62,7 +65,7 @@ struct SepCoord {
         by = ((block / ntx) % nty) * 4 * WY;
         bw = (block / (ntx * nty)) * 16;
         const int lane = tid & 31, warp = tid >> 5;
-        lw = lane >> 4; lx = (lane >> 2) & 3; ly = lane & 3;
+        lw = lane & 1; ly = (lane >> 1) & 3; lx = (lane >> 3) & 3;
         ww = warp >> 1; wx = warp & 1;
         iw0 = bw + 4 * ww + 2 * lw;
         ix0 = bx + 8 * wx + 2 * lx;
@@ -178,13 +181,10 @@ rad_sep_kernel(const MainParams P) {
     constexpr int YN = SH::YN, EV = SH::EV, S = SEP_S, NB = SEP_NB;
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *ring = reinterpret_cast<double *>(smem_raw);
-    double *Tre = reinterpret_cast<double *>(smem_raw + SH::OFF_T);       // [NB][S][256]
-    double *Tim = Tre + NB * S * 256;
-    double *Yre = reinterpret_cast<double *>(smem_raw + SH::OFF_Y);       // [NB][S][YN]
-    double *Yim = Yre + NB * S * YN;
-    double *Fx = reinterpret_cast<double *>(smem_raw + SH::OFF_F);        // [NB][S][YN]  w f_x, w f_y
-    double *Fy = Fx + NB * S * YN;
-    double *Hh = reinterpret_cast<double *>(smem_raw + SH::OFF_H);        // [NB][S][YN]  w h (spin-1/2)
+    double2 *Tt = reinterpret_cast<double2 *>(smem_raw + SH::OFF_T);      // [NB][S][256]  T = (re, im)
+    double2 *Yt = reinterpret_cast<double2 *>(smem_raw + SH::OFF_Y);      // [NB][S][YN]   Y = (re, im)
+    double2 *Ft = reinterpret_cast<double2 *>(smem_raw + SH::OFF_F);      // [NB][S][YN]   (w f_x, w f_y)
+    double *Hh = reinterpret_cast<double *>(smem_raw + SH::OFF_H);        // [NB][S][YN]   w h (spin-1/2)
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem_raw + SH::OFF_BAR);   // trajectory stages
     uint64_t *full = bars + SEP_STAGES, *empty = full + NB;
     const int tid = threadIdx.x;
@@ -208,8 +208,8 @@ rad_sep_kernel(const MainParams P) {
 #pragma unroll
         for (int r = 0; r < RT; ++r) {
             const int b = pt + r * SEP_PROD;
-            const int iw = co.bw + 4 * (b >> 6) + 2 * ((b >> 2) & 1) + ((b >> 4) & 1);
-            const int ix = co.bx + 8 * ((b >> 5) & 1) + 2 * (b & 3) + ((b >> 3) & 1);
+            const int iw = co.bw + 4 * (b >> 6) + 2 * (b & 1) + ((b >> 4) & 1);
+            const int ix = co.bx + 8 * ((b >> 5) & 1) + 2 * ((b >> 1) & 3) + ((b >> 3) & 1);
             omT[r] = P.omega[min(iw, P.n_omega - 1)];
             nxT[r] = P.thx[min(ix, P.n_thx - 1)];
         }
@@ -218,8 +218,8 @@ rad_sep_kernel(const MainParams P) {
             const int b = pt + r * SEP_PROD;
             {
                 const int q = b >> 3, m = q % WY, i = (q / WY) & 1, ww = (q / WY) >> 1;
-                const int iw = co.bw + 4 * ww + 2 * ((b >> 2) & 1) + i;
-                const int iy = co.by + WY * (b & 3) + m;
+                const int iw = co.bw + 4 * ww + 2 * (b & 1) + i;
+                const int iy = co.by + WY * ((b >> 1) & 3) + m;
                 omY[r] = P.omega[min(iw, P.n_omega - 1)];
                 nyY[r] = P.thy[min(iy, P.n_thy - 1)];
             }
@@ -296,15 +296,13 @@ rad_sep_kernel(const MainParams P) {
                     for (int r = 0; r < RT; ++r) {
                         const double dT = fma(-nxT[r], r89.x, fma(hxT[r], r67.y, r67.x));
                         const double2 ph = phasor_full(fma(whT[r], dT, p0T[r]));
-                        Tre[row * 256 + pt + r * SEP_PROD] = ph.x;
-                        Tim[row * 256 + pt + r * SEP_PROD] = ph.y;
+                        Tt[row * 256 + pt + r * SEP_PROD] = ph;
                     }
 #pragma unroll
                     for (int r = 0; r < RY; ++r) {
                         const double dY = fma(-nyY[r], r89.y, hyY[r] * r67.y);
                         const double2 ph = phasor_full(fma(whY[r], dY, p0Y[r]));
-                        Yre[row * YN + pt + r * SEP_PROD] = ph.x;
-                        Yim[row * YN + pt + r * SEP_PROD] = ph.y;
+                        Yt[row * YN + pt + r * SEP_PROD] = ph;
                     }
                     const double2 r01 = *reinterpret_cast<const double2 *>(rec);       // D0, vx
                     const double2 r23 = *reinterpret_cast<const double2 *>(rec + 2);   // vy, w ax
@@ -319,8 +317,8 @@ rad_sep_kernel(const MainParams P) {
                         const double gq = inv_square(q);
                         const double s1 = fma(nyF[r], r45.x, r45.y);
                         const double s2 = fma(nxF[r], r23.y, r45.y);
-                        Fx[row * YN + pt + r * SEP_PROD] = fma(s1, ux, -(bx * r23.y)) * gq;
-                        Fy[row * YN + pt + r * SEP_PROD] = fma(s2, uy, -(by * r45.x)) * gq;
+                        Ft[row * YN + pt + r * SEP_PROD] = make_double2(fma(s1, ux, -(bx * r23.y)) * gq,
+                                                                        fma(s2, uy, -(by * r45.x)) * gq);
                         if (NC == 6) Hh[row * YN + pt + r * SEP_PROD] = fma(nxF[r], r23.y, s1) * gq;
                     }
                 }
@@ -342,8 +340,8 @@ rad_sep_kernel(const MainParams P) {
     const SepCoord<WY> co(blockIdx.x, tid, P.n_thx, P.n_thy);
     const int64_t gid = (int64_t)blockIdx.x * SEP_CONS + tid;
     // read offsets (entries) of this thread inside one sample's tables
-    const int rT = (co.ww * 2 + co.wx) * 32 + co.lw * 4 + co.lx;          // + (i*2 + j) * 8
-    const int rY = co.ww * 2 * WY * 8 + co.lw * 4 + co.ly;                // + (i*WY + m) * 8
+    const int rT = (co.ww * 2 + co.wx) * 32 + co.lx * 2 + co.lw;          // + (i*2 + j) * 8
+    const int rY = co.ww * 2 * WY * 8 + co.ly * 2 + co.lw;                // + (i*WY + m) * 8
     const int rF = co.wx * 2 * WY * 16 + co.lx * 4 + co.ly;               // + (j*WY + m) * 16
 
     // ---- output slots of this thread: zero them, later every trajectory adds its spectrum
@@ -392,33 +390,32 @@ rad_sep_kernel(const MainParams P) {
 #pragma unroll
         for (int s = 0; s < S; ++s) {                 // a4: complex multiply + accumulate
             const int row = buf * S + s;
-            const double *tre = Tre + row * 256 + rT, *tim = Tim + row * 256 + rT;
-            const double *yre = Yre + row * YN + rY, *yim = Yim + row * YN + rY;
-            const double *fxp = Fx + row * YN + rF, *fyp = Fy + row * YN + rF, *hp = Hh + row * YN + rF;
-            double tr[2][2], ti[2][2];
+            const double2 *tp = Tt + row * 256 + rT, *yp = Yt + row * YN + rY, *fp = Ft + row * YN + rF;
+            const double *hp = Hh + row * YN + rF;
+            double2 tv[2][2];
 #pragma unroll
             for (int i = 0; i < 2; ++i)
 #pragma unroll
-                for (int j = 0; j < 2; ++j) { tr[i][j] = tre[(i * 2 + j) * 8]; ti[i][j] = tim[(i * 2 + j) * 8]; }
+                for (int j = 0; j < 2; ++j) tv[i][j] = tp[(i * 2 + j) * 8];
 #pragma unroll
             for (int m = 0; m < WY; ++m) {
-                double yr[2], yi[2];
+                double2 yv[2];
 #pragma unroll
-                for (int i = 0; i < 2; ++i) { yr[i] = yre[(i * WY + m) * 8]; yi[i] = yim[(i * WY + m) * 8]; }
+                for (int i = 0; i < 2; ++i) yv[i] = yp[(i * WY + m) * 8];
 #pragma unroll
                 for (int j = 0; j < 2; ++j) {
-                    const double fxv = fxp[(j * WY + m) * 16], fyv = fyp[(j * WY + m) * 16];
+                    const double2 f = fp[(j * WY + m) * 16];
                     double hv = 0.0;
                     if (NC == 6) hv = hp[(j * WY + m) * 16];
 #pragma unroll
                     for (int i = 0; i < 2; ++i) {
-                        const double qr = fma(-ti[i][j], yi[i], tr[i][j] * yr[i]);
-                        const double qi = fma(ti[i][j], yr[i], tr[i][j] * yi[i]);
+                        const double qr = fma(-tv[i][j].y, yv[i].y, tv[i][j].x * yv[i].x);
+                        const double qi = fma(tv[i][j].y, yv[i].x, tv[i][j].x * yv[i].y);
                         double *a = acc[(i * 2 + j) * WY + m];
-                        a[0] = fma(fxv, qr, a[0]);
-                        a[1] = fma(fxv, qi, a[1]);
-                        a[2] = fma(fyv, qr, a[2]);
-                        a[3] = fma(fyv, qi, a[3]);
+                        a[0] = fma(f.x, qr, a[0]);
+                        a[1] = fma(f.x, qi, a[1]);
+                        a[2] = fma(f.y, qr, a[2]);
+                        a[3] = fma(f.y, qi, a[3]);
                         if (NC == 6) {
                             a[4] = fma(hv, qr, a[4]);
                             a[5] = fma(hv, qi, a[5]);

@@ -151,7 +151,11 @@ def test_deterministic(rad):
 def test_direct_mode_many_tiles(rad, oracle_mod):
     """Grid large enough (>= 8 CTAs per SM) for the no-split path; sampled + lattice."""
     wl = workloads.make("cfg2", n=300, n_omega=40, n_th=200, seed=21)
-    cube = run_single(rad, wl, CL, 0.0)
+    rad.rad_set_kernel(1)                              # the direct-phasor kernel (auto would pick the separable one)
+    try:
+        cube = run_single(rad, wl, CL, 0.0)
+    finally:
+        rad.rad_set_kernel(0)
     idx, ref = sampled_reference(oracle_mod, wl, cube, 3000, (5, 9, 9), CL, 0.0)
     assert_parity(cube, ref, idx, label="direct")
 
@@ -253,24 +257,36 @@ def test_angular_sum(rad):
 
 
 # ------------------------------------------------------------------ full-size configs, sampled
-def test_cfg2_full_size_sampled(rad, oracle_mod):
+@pytest.fixture(params=[0, 1, 2], ids=["auto", "direct", "separable"])
+def each_kernel(request, rad):
+    """The full-size configs run through the kernel the library picks (what bench.py times) and through
+    each of the two kernels forced (include/rad.h rad_set_kernel)."""
+    rad.rad_set_kernel(request.param)
+    yield rad
+    rad.rad_set_kernel(0)
+
+
+def test_cfg2_full_size_sampled(each_kernel, oracle_mod):
     """BASELINE.json configs[1] at full size, in the launch configuration bench.py times."""
+    rad = each_kernel
     wl = workloads.make("cfg2")
     cube = run_single(rad, wl, CL, 0.0)
     idx, ref = sampled_reference(oracle_mod, wl, cube, 3000, (8, 6, 6), CL, 0.0)
     assert_parity(cube, ref, idx, label="cfg2 full")
 
 
-def test_cfg3_full_size_sampled(rad, oracle_mod):
+def test_cfg3_full_size_sampled(each_kernel, oracle_mod):
     """BASELINE.json configs[2]: spin-1/2, N = 2e5, |phase| up to ~1e6 rad; 512 x 64 x 64 grid."""
+    rad = each_kernel
     wl = workloads.make("cfg3")
     cube = run_single(rad, wl, SH, wl.hbarc_over_E)
     idx, ref = sampled_reference(oracle_mod, wl, cube, 160, (4, 3, 3), SH, wl.hbarc_over_E)
     assert_parity(cube, ref, idx, label="cfg3 full")
 
 
-def test_cfg4_reduced_ensemble_sampled(rad, oracle_mod):
+def test_cfg4_reduced_ensemble_sampled(each_kernel, oracle_mod):
     """configs[3] shape (128 x 16 x 16 grid, batched trajectories) with 48 x 20000 samples."""
+    rad = each_kernel
     we = workloads.make("cfg4", count=48, n=20000)
     cube = rad.rad_ensemble_sum(dev_dict(we.batch), we.n, *dev_grid(we)).cpu().numpy()
     idx = workloads.sample_points(we, 100, (4, 3, 3))
@@ -281,8 +297,9 @@ def test_cfg4_reduced_ensemble_sampled(rad, oracle_mod):
 
 
 @pytest.mark.parametrize("model", [S0, SH])
-def test_cfg5_reduced_sampled(rad, oracle_mod, model):
+def test_cfg5_reduced_sampled(each_kernel, oracle_mod, model):
     """configs[4] (axial well, both spin variants) at N = 2e5 on the full 1024 x 64 x 64 grid."""
+    rad = each_kernel
     wl = workloads.make("cfg5", n=200000, model=model)
     cube = run_single(rad, wl, model, wl.hbarc_over_E)
     idx, ref = sampled_reference(oracle_mod, wl, cube, 120, (4, 3, 3), model, wl.hbarc_over_E)
