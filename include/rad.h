@@ -31,8 +31,10 @@
  *   - `workspace` is caller-owned DEVICE scratch of at least rad_workspace_bytes()
  *     bytes, 256-byte aligned.  If NULL, scratch is taken from the device's
  *     stream-ordered pool (cudaMallocAsync / cudaFreeAsync on `cuda_stream`) and
- *     released in stream order.  The library keeps no pointer past the enqueued work
- *     and allocates nothing persistent.
+ *     released in stream order; the first such call raises that pool's release threshold
+ *     (cudaMemPoolAttrReleaseThreshold) so that freed scratch stays cached in the pool instead
+ *     of going back to the driver at every synchronisation.  The library keeps no pointer past
+ *     the enqueued work and allocates nothing persistent of its own.
  *   - `cuda_stream` is a cudaStream_t (NULL = legacy default stream).  All work is
  *     enqueued on it; no call synchronises the host (the *_host calls do, once, at
  *     the end).
@@ -152,6 +154,10 @@ int64_t rad_launch_count(void);
  * wastes less than half of the work, else the direct kernel (one phasor per eval).  1: always direct,
  * 2: always separable.  Both meet the same tolerance; process-wide; RAD_EINVAL on other values. */
 int rad_set_kernel(int choice);
+
+/* Which kernel a call on a grid of this shape uses under the current rad_set_kernel setting:
+ * 1 direct, 2 separable (a pure function of the arguments; no device needed); RAD_EINVAL on bad input. */
+int rad_plan_kernel(int32_t n_omega, int32_t n_thx, int32_t n_thy, rad_model model);
 
 /* Per-kernel timing of the most recent device-buffer call (for the roofline in bench.py).
  * rad_profile_enable(1) makes every later call record CUDA events on its stream around the

@@ -19,7 +19,7 @@ FIELDS = ("t", "dz", "x", "y", "vx", "vy", "dvz", "ax", "ay", "az", "gamma")
 EXPORTS = ("rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_angular_sum", "rad_sum_cubes",
            "rad_workspace_bytes", "rad_eval_host", "rad_ensemble_sum_host",
            "rad_measure_fp64_peak", "rad_launch_count", "rad_strerror",
-           "rad_profile_enable", "rad_profile_last", "rad_set_kernel")
+           "rad_profile_enable", "rad_profile_last", "rad_set_kernel", "rad_plan_kernel")
 
 _dp = ctypes.POINTER(ctypes.c_double)
 _lib = None
@@ -301,6 +301,17 @@ def rad_set_kernel(choice: int = 0) -> None:
     lib.rad_set_kernel.argtypes = [ctypes.c_int]
     lib.rad_set_kernel.restype = ctypes.c_int
     _check(lib.rad_set_kernel(int(choice)))
+
+
+def rad_plan_kernel(n_omega: int, n_thx: int, n_thy: int, model: int = CLASSICAL) -> int:
+    """1: direct-phasor kernel, 2: separable-phasor kernel, for a grid of this shape (current setting)."""
+    lib = load_library()
+    lib.rad_plan_kernel.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int]
+    lib.rad_plan_kernel.restype = ctypes.c_int
+    rc = lib.rad_plan_kernel(n_omega, n_thx, n_thy, int(model))
+    if rc < 0:
+        _check(rc)
+    return rc
 
 
 def rad_profile_enable(on: bool = True) -> None:

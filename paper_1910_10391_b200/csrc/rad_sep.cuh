@@ -22,7 +22,7 @@
 //               address are merged (measured), so l_w is the lowest lane bit -- the
 //               F table (8 entries per thread, independent of omega) then costs half.
 // full[] / empty[] mbarriers hand table buffers over; setmaxnreg moves registers from the
-// producers (104) to the consumers (200), whose accumulators need them.
+// producers to the consumers, whose accumulators need them (SepRegs).
 #pragma once
 
 namespace rad {
@@ -30,13 +30,35 @@ namespace rad {
 constexpr int SEP_CONS = 256;  // consumer threads
 constexpr int SEP_PROD = 128;  // producer threads
 constexpr int SEP_T = SEP_CONS + SEP_PROD;
-constexpr int SEP_S = 4;       // samples per table sub-block
-constexpr int SEP_NB = 3;      // table buffers in flight
+#ifndef RAD_SEP_S
+#define RAD_SEP_S 8
+#endif
+#ifndef RAD_SEP_NB
+#define RAD_SEP_NB 2
+#endif
+#ifndef RAD_SEP_DEG
+#define RAD_SEP_DEG 5          // polynomial set of the table phasors (sincos_coeffs.h): 5 = 1e-13 (as the direct kernel), 6 = 2e-16
+#endif
+#ifndef RAD_SEP_REGS_CONS4          // registers per consumer thread after setmaxnreg, 4 / 6 accumulators per point
+#define RAD_SEP_REGS_CONS4 192
+#endif
+#ifndef RAD_SEP_REGS_CONS6
+#define RAD_SEP_REGS_CONS6 200
+#endif
+constexpr int SEP_S = RAD_SEP_S;       // samples per table sub-block
+constexpr int SEP_NB = RAD_SEP_NB;     // table buffers in flight
 constexpr int SEP_STAGES = 3;  // trajectory-chunk ring depth
 constexpr int SEP_REGS_LAUNCH = 168;                         // __launch_bounds__(384, 1): 65536 / 384 rounded down to 8
-constexpr int SEP_REGS_CONS = 200, SEP_REGS_PROD = 104;          // 256 * 200 + 128 * 104 = 384 * 168: the pool the CTA got at launch
-static_assert(SEP_CONS * SEP_REGS_CONS + SEP_PROD * SEP_REGS_PROD <= SEP_T * SEP_REGS_LAUNCH,
-              "setmaxnreg.inc would wait forever for registers the CTA does not own");
+// setmaxnreg moves registers between the roles inside the pool the CTA got at launch (384 * 168):
+// 256 * CONS + 128 * PROD <= 384 * 168, both multiples of 8.  Measured best splits: 192 / 120 with
+// 4 accumulators per point (the producers build 6 table entries per sample and need the room),
+// 200 / 104 with 6 (the producers build 4, the consumers carry the J accumulators).
+template <int NC> struct SepRegs {
+    static constexpr int CONS = NC == 6 ? RAD_SEP_REGS_CONS6 : RAD_SEP_REGS_CONS4;
+    static constexpr int PROD = ((SEP_T * SEP_REGS_LAUNCH - SEP_CONS * CONS) / SEP_PROD) / 8 * 8;
+    static_assert(CONS % 8 == 0 && PROD >= 24 && SEP_CONS * CONS + SEP_PROD * PROD <= SEP_T * SEP_REGS_LAUNCH,
+                  "setmaxnreg.inc would wait forever for registers the CTA does not own");
+};
 
 template <int NC, int WY>
 struct SepShape {
@@ -87,10 +109,10 @@ __device__ __forceinline__ dd half_square_dd(double a) {      // a^2 / 2
     return {0.5 * s.hi, 0.5 * s.lo};
 }
 
-// true (cos, sin) of 2 pi p, high-accuracy polynomial set (tables are built once per 16 evals)
+// true (cos, sin) of 2 pi p
 __device__ __forceinline__ double2 phasor_full(double p) {
     double c, s;
-    phasor_turns<6>(p, c, s);
+    phasor_turns<RAD_SEP_DEG>(p, c, s);
     return make_double2(c, s * 1.4142135623730951);
 }
 
@@ -199,7 +221,7 @@ rad_sep_kernel(const MainParams P) {
 
     if (tid >= SEP_CONS) {
         // ====================================================================== PRODUCERS (phase A)
-        reg_dealloc<SEP_REGS_PROD>();
+        reg_dealloc<SepRegs<NC>::PROD>();
         const int pt = tid - SEP_CONS;
         const int tile_bx = blockIdx.x;
         const SepCoord<WY> co(tile_bx, 0, P.n_thx, P.n_thy);             // tile bases only
@@ -336,7 +358,7 @@ rad_sep_kernel(const MainParams P) {
     }
 
     // ========================================================================== CONSUMERS (phase B)
-    reg_alloc<SEP_REGS_CONS>();
+    reg_alloc<SepRegs<NC>::CONS>();
     const SepCoord<WY> co(blockIdx.x, tid, P.n_thx, P.n_thy);
     const int64_t gid = (int64_t)blockIdx.x * SEP_CONS + tid;
     // read offsets (entries) of this thread inside one sample's tables
