@@ -41,10 +41,11 @@ UNIT = "evals/s"
 # against ncu's 2*DFMA + DMUL + DADD count (45.6 on cfg2).  SURVEY.md 8(d) estimated 52-60.
 # The separable-phasor kernel needs far fewer: per eval one complex multiply (6) and
 # the accumulation (8 [12]), plus per 16 [8] evals one T and one [half a] Y phasor and one [half an]
-# integrand entry (42 + 41 + 28 [31] flops) -> 20.9 [27.8]; ncu counts 12.1 FP64 instructions per eval.
+# integrand entry (38 + 37 + 28 [31] flops) -> 20.44 [27.0] flops, 12.0 [15.56] FP64 instructions;
+# ncu counts 11.9 [15.5] instructions per eval.
 KERNELS = {1: "rad_main_kernel (direct phasor)", 2: "rad_sep_kernel (separable phasor)"}
-FLOPS_PER_EVAL = {1: {0: 45.25, 1: 45.25, 2: 49.6}, 2: {0: 20.94, 1: 20.94, 2: 27.75}}
-FP64_INSTR_PER_EVAL = {1: {0: 26.6, 1: 26.6, 2: 28.9}, 2: {0: 12.25, 1: 12.25, 2: 15.94}}
+FLOPS_PER_EVAL = {1: {0: 45.25, 1: 45.25, 2: 49.6}, 2: {0: 20.44, 1: 20.44, 2: 27.0}}
+FP64_INSTR_PER_EVAL = {1: {0: 26.6, 1: 26.6, 2: 28.9}, 2: {0: 12.0, 1: 12.0, 2: 15.56}}
 FP64_SPEC_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # 148 SM x 64 FMA lanes x 2 x 1.965 GHz
 
 

@@ -669,8 +669,8 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const rad_g
     prof_mark(2, st);
     if (pl.mode != MODE_DIRECT) {
         if (pl.kernel == 1) {
-            if (nc == 6) rad_sep_finalize_kernel<6, 2><<<pl.tiles, SEP_CONS, 0, st>>>(mp);
-            else rad_sep_finalize_kernel<4, 4><<<pl.tiles, SEP_CONS, 0, st>>>(mp);
+            if (nc == 6) rad_sep_finalize_kernel<6, 2><<<dim3(pl.tiles, 8), SEP_CONS, 0, st>>>(mp);
+            else rad_sep_finalize_kernel<4, 4><<<dim3(pl.tiles, 16), SEP_CONS, 0, st>>>(mp);
         } else {
             if (nc == 6) rad_finalize_kernel<6><<<pl.tiles, TPB, 0, st>>>(mp);
             else rad_finalize_kernel<4><<<pl.tiles, TPB, 0, st>>>(mp);

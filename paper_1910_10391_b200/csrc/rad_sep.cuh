@@ -490,10 +490,11 @@ rad_sep_finalize_kernel(const MainParams P) {
     const SepCoord<WY> co(blockIdx.x, threadIdx.x, P.n_thx, P.n_thy);
     const int64_t gid = (int64_t)blockIdx.x * SEP_CONS + threadIdx.x;
     const int A = P.n_thx * P.n_thy;
-    for (int e = 0; e < EV; ++e) {
+    {                                                 // gridDim.y = EV: one of the thread's points per CTA row
+        const int e = blockIdx.y;
         const int m = e % WY, j = (e / WY) & 1, i = e / (2 * WY);
         const int iw = co.iw0 + i, ix = co.ix0 + j, iy = co.iy0 + m;
-        if (iw >= P.n_omega || ix >= P.n_thx || iy >= P.n_thy) continue;
+        if (iw >= P.n_omega || ix >= P.n_thx || iy >= P.n_thy) return;
         double total = 0.0;
         if (P.mode == MODE_PSLICE) {
             for (int s = 0; s < P.p_slices; ++s)                       // slices ascending
