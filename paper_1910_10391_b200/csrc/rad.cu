@@ -506,15 +506,27 @@ static Plan make_plan(int count, int64_t n_max, int n_omega, int n_thx, int n_th
         pl.tiles = (int)((T + TPB - 1) / TPB);
         pl.t_pad = (int64_t)pl.tiles * TPB;
         per_thread_p = W; per_thread_t = (size_t)nc * W;
-        const int target = sms * 8;                   // CTAs wanted in flight over the launch
-        if (pl.tiles < target) {
-            const int want = (target + pl.tiles - 1) / pl.tiles;       // slices wanted per tile
-            if (count >= want) { pl.mode = MODE_PSLICE; pl.p_slices = want; }
-            else if (count > 1 || want > 1) {
-                int ts = (want + count - 1) / count;
-                ts = std::min(ts, std::max(1, pl.cpt / 2));            // >= 2 chunks per slice
-                if (ts > 1) { pl.mode = MODE_TSPLIT; pl.t_slices = ts; pl.p_slices = count; }
-                else if (count > 1) { pl.mode = MODE_PSLICE; pl.p_slices = count; }
+        // two CTAs per SM: the fewest slices k (>= 2 waves of work) whose tiles*k CTAs fill whole
+        // waves of 2 * sms to >= 98.5 %
+        const int slots = 2 * sms;
+        if (pl.tiles < 8 * sms) {
+            const int64_t kmax = std::max<int64_t>(1, (int64_t)count * std::max(1, pl.cpt / 2));
+            int best_k = 1;
+            double best = 0.0;
+            for (int64_t k = 1; k <= std::min<int64_t>(kmax, 8 * sms); ++k) {
+                const int64_t ctas = (int64_t)pl.tiles * k;
+                double eff = (double)ctas / (double)((ctas + slots - 1) / slots * slots);
+                if (ctas < 2 * slots && k < kmax) eff *= 0.5;        // too few CTAs to balance: keep looking
+                if (eff > best + 1e-9) { best = eff; best_k = (int)k; }
+                if (eff >= 0.985) break;
+            }
+            if (best_k > 1) {
+                if (count >= best_k) { pl.mode = MODE_PSLICE; pl.p_slices = best_k; }
+                else {
+                    int ts = std::min((best_k + count - 1) / count, std::max(1, pl.cpt / 2));
+                    if (ts > 1) { pl.mode = MODE_TSPLIT; pl.t_slices = ts; pl.p_slices = count; }
+                    else if (count > 1) { pl.mode = MODE_PSLICE; pl.p_slices = count; }
+                }
             }
         }
     } else {
