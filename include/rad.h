@@ -111,6 +111,18 @@ int rad_ensemble_sum(const rad_traj_batch *batch, const rad_grid *grid, rad_mode
                      const double *hbarc_over_E, int accumulate, double *out,
                      void *workspace, size_t workspace_bytes, void *cuda_stream);
 
+/* One long trajectory cut into sections with their own energy -- the paper's treatment of energy
+ * loss: "the total spectrum is then the sum of the spectra from each section".
+ * out[m] (+)= sum over s (ascending) of the spectrum of samples start[s] .. start[s+1], BOTH included:
+ * neighbouring sections share their boundary sample, so their trapezoid weights tile the time axis.
+ * start: HOST array of n_sections + 1 strictly ascending sample indices in [0, traj->n - 1];
+ * hbarc_over_E: HOST array, one per section (NULL allowed iff classical); the J coefficient of
+ * eq. (10) uses gamma of each section's first sample.  Choosing the sections (each longer than the
+ * formation length l_f = 2 gamma^2 (E - w)/(E w)) is the caller's business: not checked. */
+int rad_sections_sum(const rad_traj *traj, int32_t n_sections, const int64_t *start, const rad_grid *grid,
+                     rad_model model, const double *hbarc_over_E, int accumulate, double *out,
+                     void *workspace, size_t workspace_bytes, void *cuda_stream);
+
 /* dI/dw[i_w] = sum_{i_x,i_y} cube * d_omega_solid, optionally only where
  * n_x^2 + n_y^2 <= theta_cut^2 (theta_cut <= 0: no mask) -- the paper's "final sum over
  * the spatial integrals", done on the device.  `cube` is the output of

@@ -6,7 +6,8 @@ memory and streams.  There is no CPU fallback: if the shared library is missing 
 no CUDA device is visible, calls raise.
 
 Functions mirror the C entry points one to one:
-``rad_classical``, ``rad_semiclassical``, ``rad_ensemble_sum``, ``rad_angular_sum``, ``rad_sum_cubes``,
+``rad_classical``, ``rad_semiclassical``, ``rad_ensemble_sum``, ``rad_sections_sum``, ``rad_angular_sum``,
+``rad_sum_cubes``,
 ``rad_workspace_bytes``, ``rad_eval_host``, ``rad_ensemble_sum_host``,
 ``rad_measure_fp64_peak``, ``rad_launch_count``.
 """
@@ -16,13 +17,13 @@ from .binding import (CLASSICAL, FIELDS, SPIN0, SPIN_HALF, RadError, build_libra
                       load_library, rad_angular_sum, rad_classical, rad_ensemble_sum,
                       rad_ensemble_sum_host, rad_eval_host, rad_launch_count,
                       rad_measure_fp64_peak, rad_profile_enable, rad_profile_last,
-                      rad_plan_kernel, rad_semiclassical, rad_set_kernel, rad_sum_cubes, rad_workspace_bytes)
+                      rad_plan_kernel, rad_sections_sum, rad_semiclassical, rad_set_kernel, rad_sum_cubes, rad_workspace_bytes)
 from .sharding import rad_ensemble_sum_sharded, rad_eval_grid_sharded, shard_range, shard_sizes
 
 __all__ = [
     "CLASSICAL", "SPIN0", "SPIN_HALF", "FIELDS", "RadError", "build_library", "library_path",
     "load_library", "rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_angular_sum",
     "rad_workspace_bytes", "rad_eval_host", "rad_ensemble_sum_host", "rad_measure_fp64_peak",
-    "rad_launch_count", "rad_profile_enable", "rad_profile_last", "rad_sum_cubes", "rad_set_kernel", "rad_plan_kernel",
+    "rad_launch_count", "rad_profile_enable", "rad_profile_last", "rad_sum_cubes", "rad_set_kernel", "rad_plan_kernel", "rad_sections_sum",
     "rad_ensemble_sum_sharded", "rad_eval_grid_sharded", "shard_range", "shard_sizes",
 ]

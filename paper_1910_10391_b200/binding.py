@@ -16,7 +16,7 @@ _SO = _PKG / "librad_b200.so"
 CLASSICAL, SPIN0, SPIN_HALF = 0, 1, 2
 FIELDS = ("t", "dz", "x", "y", "vx", "vy", "dvz", "ax", "ay", "az", "gamma")
 
-EXPORTS = ("rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_angular_sum", "rad_sum_cubes",
+EXPORTS = ("rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_sections_sum", "rad_angular_sum", "rad_sum_cubes",
            "rad_workspace_bytes", "rad_eval_host", "rad_ensemble_sum_host",
            "rad_measure_fp64_peak", "rad_launch_count", "rad_strerror",
            "rad_profile_enable", "rad_profile_last", "rad_set_kernel", "rad_plan_kernel")
@@ -81,6 +81,9 @@ def load_library() -> ctypes.CDLL:
                                       vp, vp, sz, vp]
     lib.rad_ensemble_sum.argtypes = [ctypes.POINTER(_Batch), ctypes.POINTER(_Grid), ctypes.c_int, vp,
                                      ctypes.c_int, vp, vp, sz, vp]
+    lib.rad_sections_sum.argtypes = [ctypes.POINTER(_Traj), i32, vp, ctypes.POINTER(_Grid), ctypes.c_int, vp,
+                                     ctypes.c_int, vp, vp, sz, vp]
+    lib.rad_sections_sum.restype = ctypes.c_int
     lib.rad_angular_sum.argtypes = [vp, ctypes.POINTER(_Grid), dbl, dbl, vp, vp]
     lib.rad_sum_cubes.argtypes = [vp, i32, i64, ctypes.c_int, vp, vp]
     lib.rad_workspace_bytes.argtypes = [i32, i64, i32, i32, i32]
@@ -204,6 +207,28 @@ def rad_ensemble_sum(batch: dict, n, omega, thx, thy, model: int = CLASSICAL, hb
                                            lam.ctypes.data if lam is not None else None,
                                            1 if accumulate else 0, out.data_ptr(), ws, nb,
                                            _stream_ptr(stream)))
+    return out
+
+
+def rad_sections_sum(traj: dict, start, omega, thx, thy, model: int = CLASSICAL, hbarc_over_E=None,
+                     accumulate: bool = False, out=None, workspace=None, stream=None):
+    """Sum of the spectra of the sections start[s]..start[s+1] (both included) of one trajectory, each with
+    its own hbar c / E."""
+    t = _traj_struct(traj)
+    st = np.ascontiguousarray(start, dtype=np.int64)
+    if st.ndim != 1 or st.size < 2:
+        raise ValueError("start needs at least two indices")
+    lam = None
+    if hbarc_over_E is not None:
+        lam = np.ascontiguousarray(np.broadcast_to(np.asarray(hbarc_over_E, dtype=np.float64), (st.size - 1,)))
+    g = _grid_struct(_dev(omega, "omega"), _dev(thx, "thx"), _dev(thy, "thy"))
+    if accumulate and out is None:
+        raise ValueError("accumulate needs an existing out")
+    out = _out_cube(out, omega, thx, thy)
+    ws, nb = _ws_args(workspace)
+    _check(load_library().rad_sections_sum(ctypes.byref(t), st.size - 1, st.ctypes.data, ctypes.byref(g), int(model),
+                                           lam.ctypes.data if lam is not None else None,
+                                           1 if accumulate else 0, out.data_ptr(), ws, nb, _stream_ptr(stream)))
     return out
 
 

@@ -75,7 +75,8 @@ __device__ __forceinline__ dd phase_offset_dd(double gamma, double t, double dz,
 }
 
 __global__ void __launch_bounds__(256)
-rad_pack_kernel(rad_traj_batch b, const int64_t *n_dev, int64_t n_single, int cpt, double *packed) {
+rad_pack_kernel(rad_traj_batch b, const int64_t *n_dev, int64_t n_single, const int64_t *off_dev, int cpt,
+                double *packed) {
     const int p = blockIdx.y;
     const int64_t slot = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (slot >= (int64_t)cpt * CH) return;
@@ -83,7 +84,7 @@ rad_pack_kernel(rad_traj_batch b, const int64_t *n_dev, int64_t n_single, int cp
     const int c = (int)(slot / CH), i = (int)(slot % CH);
     const int64_t c0 = (int64_t)c * CH;
     if (c0 >= n) return;                              // chunk never read
-    const int64_t o = (int64_t)p * b.stride;
+    const int64_t o = off_dev ? off_dev[p] : (int64_t)p * b.stride;     // first sample of trajectory / section p
     const int nvalid = (int)min((int64_t)CH, n - c0);
     const int64_t kb = c0 + min(CH / 2, nvalid - 1);  // base sample of the chunk
     double *chunk = packed + ((int64_t)p * cpt + c) * CHUNK_DBL;
@@ -476,7 +477,7 @@ struct Plan {
     int kernel;               // 0: rad_main_kernel (one phasor per eval), 1: rad_sep_kernel (separable phasor)
     int cpt, tiles, p_slices, t_slices, mode;
     int64_t t_pad;
-    size_t off_packed, off_n, off_lam, off_partial, total;
+    size_t off_packed, off_n, off_lam, off_start, off_partial, total;
 };
 
 static std::atomic<int> g_kernel_choice{0};          // rad_set_kernel: 0 auto, 1 direct, 2 separable
@@ -559,6 +560,7 @@ static Plan make_plan(int count, int64_t n_max, int n_omega, int n_thx, int n_th
     pl.off_packed = off; off += align_up((size_t)count * pl.cpt * CHUNK_BYTES, 256);
     pl.off_n = off;      off += align_up((size_t)count * sizeof(int64_t), 256);
     pl.off_lam = off;    off += align_up((size_t)count * sizeof(double), 256);
+    pl.off_start = off;  off += align_up((size_t)count * sizeof(int64_t), 256);
     pl.off_partial = off;
     if (pl.mode == MODE_PSLICE) off += align_up((size_t)pl.p_slices * per_thread_p * pl.t_pad * 8, 256);
     if (pl.mode == MODE_TSPLIT) off += align_up((size_t)count * pl.t_slices * per_thread_t * pl.t_pad * 8, 256);
@@ -600,8 +602,10 @@ static cudaError_t launch_sep(const MainParams &mp, dim3 grid, cudaStream_t st) 
 }
 
 // Everything: pack, main, finalize.  All device pointers; n_host / lam_host are host arrays.
-static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const rad_grid *g, int model,
-                     const double *lam_host, int accumulate, double *out,
+// off_host (optional): first sample of each trajectory inside the arrays (sections of one long trajectory);
+// NULL: row p starts at p * stride.
+static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const int64_t *off_host, const rad_grid *g,
+                     int model, const double *lam_host, int accumulate, double *out,
                      void *workspace, size_t workspace_bytes, cudaStream_t st) {
     if (!b || b->count < 1 || !n_host || !grid_ok(g) || !out) return RAD_EINVAL;
     if (model < RAD_CLASSICAL || model > RAD_SPIN_HALF) return RAD_EINVAL;
@@ -613,6 +617,7 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const rad_g
     int64_t n_max = 0;
     for (int p = 0; p < b->count; ++p) {
         if (n_host[p] < 2 || n_host[p] > b->stride) return RAD_EINVAL;
+        if (off_host && (off_host[p] < 0 || off_host[p] + n_host[p] > b->stride)) return RAD_EINVAL;
         n_max = std::max(n_max, n_host[p]);
         if (model != RAD_CLASSICAL && !(lam_host[p] >= 0.0)) return RAD_EDOMAIN;
     }
@@ -645,6 +650,11 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const rad_g
     double *packed = reinterpret_cast<double *>(ws + pl.off_packed);
     int64_t *n_dev = nullptr;
     double *lam_dev = nullptr;
+    int64_t *off_dev = nullptr;
+    if (off_host) {
+        off_dev = reinterpret_cast<int64_t *>(ws + pl.off_start);
+        CK(cudaMemcpyAsync(off_dev, off_host, (size_t)b->count * sizeof(int64_t), cudaMemcpyHostToDevice, st));
+    }
     if (b->count > 1) {
         n_dev = reinterpret_cast<int64_t *>(ws + pl.off_n);
         CK(cudaMemcpyAsync(n_dev, n_host, (size_t)b->count * sizeof(int64_t), cudaMemcpyHostToDevice, st));
@@ -656,7 +666,7 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const rad_g
     prof_mark(0, st);
     {   // a0/a1: pack
         dim3 grid((unsigned)(((int64_t)pl.cpt * CH + 255) / 256), (unsigned)b->count);
-        rad_pack_kernel<<<grid, 256, 0, st>>>(*b, n_dev, n_host[0], pl.cpt, packed);
+        rad_pack_kernel<<<grid, 256, 0, st>>>(*b, n_dev, n_host[0], off_dev, pl.cpt, packed);
         ++g_launches;
         CK(cudaGetLastError());
     }
@@ -701,7 +711,7 @@ static int run_single(const rad_traj *t, const rad_grid *g, int model, double la
     rad_traj_batch b{1, t->n, nullptr, t->t, t->dz, t->x, t->y, t->vx, t->vy, t->dvz,
                      t->ax, t->ay, t->az, t->gamma};
     const int64_t n = t->n;
-    return run_batch(&b, &n, g, model, &lam, 0, out, ws, ws_bytes, st);
+    return run_batch(&b, &n, nullptr, g, model, &lam, 0, out, ws, ws_bytes, st);
 }
 
 }  // namespace rad
@@ -729,7 +739,23 @@ int rad_ensemble_sum(const rad_traj_batch *batch, const rad_grid *grid, rad_mode
                      const double *hbarc_over_E, int accumulate, double *out,
                      void *workspace, size_t workspace_bytes, void *cuda_stream) {
     if (!batch) return RAD_EINVAL;
-    return run_batch(batch, batch->n, grid, (int)model, hbarc_over_E, accumulate, out,
+    return run_batch(batch, batch->n, nullptr, grid, (int)model, hbarc_over_E, accumulate, out,
+                     workspace, workspace_bytes, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int rad_sections_sum(const rad_traj *traj, int32_t n_sections, const int64_t *start, const rad_grid *grid,
+                     rad_model model, const double *hbarc_over_E, int accumulate, double *out,
+                     void *workspace, size_t workspace_bytes, void *cuda_stream) {
+    if (!traj || !start || n_sections < 1) return RAD_EINVAL;
+    std::vector<int64_t> n(n_sections), off(n_sections);
+    for (int s = 0; s < n_sections; ++s) {            // section s = samples start[s] .. start[s+1], both included
+        if (start[s] < 0 || start[s + 1] <= start[s] || start[s + 1] > traj->n - 1) return RAD_EINVAL;
+        off[s] = start[s];
+        n[s] = start[s + 1] - start[s] + 1;
+    }
+    rad_traj_batch b{n_sections, traj->n, n.data(), traj->t, traj->dz, traj->x, traj->y, traj->vx, traj->vy,
+                     traj->dvz, traj->ax, traj->ay, traj->az, traj->gamma};
+    return run_batch(&b, n.data(), off.data(), grid, (int)model, hbarc_over_E, accumulate, out,
                      workspace, workspace_bytes, static_cast<cudaStream_t>(cuda_stream));
 }
 
@@ -789,7 +815,7 @@ int rad_ensemble_sum_host(const rad_traj_batch *b, const rad_grid *g, rad_model 
     if (accumulate) CK(cudaMemcpyAsync(dout, out, M * sizeof(double), cudaMemcpyHostToDevice, st));
     rad_traj_batch db{b->count, b->stride, b->n, d[0], d[1], d[2], d[3], d[4], d[5], d[6], d[7], d[8], d[9], d[10]};
     rad_grid dg{g->n_omega, g->n_thx, g->n_thy, gw, gx, gy};
-    int rc = run_batch(&db, b->n, &dg, (int)model, hbarc_over_E, accumulate, dout, nullptr, 0, st);
+    int rc = run_batch(&db, b->n, nullptr, &dg, (int)model, hbarc_over_E, accumulate, dout, nullptr, 0, st);
     if (rc == RAD_OK) {
         cudaError_t e = cudaMemcpyAsync(out, dout, M * sizeof(double), cudaMemcpyDeviceToHost, st);
         if (e != cudaSuccess) rc = cuda_fail(e, "D2H");

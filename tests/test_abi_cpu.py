@@ -86,6 +86,14 @@ def test_validation_happens_before_any_cuda_call(radlib):
     n[1] = 8
     assert lib.rad_ensemble_sum(ctypes.byref(batch), ctypes.byref(grid), 2, None, 0, out, None, 0, None) == -1
     assert lib.rad_angular_sum(None, ctypes.byref(grid), 1.0, 0.0, out, None) == -1
+    start = np.array([0, 4, 4], dtype=np.int64)                       # empty section
+    assert lib.rad_sections_sum(ctypes.byref(traj), 2, start.ctypes.data, ctypes.byref(grid), 0, None, 0, out,
+                                None, 0, None) == -1
+    start = np.array([0, 4, 8], dtype=np.int64)                       # runs past the last sample (n = 8)
+    assert lib.rad_sections_sum(ctypes.byref(traj), 2, start.ctypes.data, ctypes.byref(grid), 0, None, 0, out,
+                                None, 0, None) == -1
+    assert lib.rad_sections_sum(ctypes.byref(traj), 0, start.ctypes.data, ctypes.byref(grid), 0, None, 0, out,
+                                None, 0, None) == -1
 
 
 def test_no_cpu_fallback(radlib):
@@ -101,3 +109,16 @@ def test_no_cpu_fallback(radlib):
         radlib.rad_classical({k: torch.zeros(8, dtype=torch.float64) for k in radlib.FIELDS},
                              torch.ones(2, dtype=torch.float64), torch.zeros(2, dtype=torch.float64),
                              torch.zeros(2, dtype=torch.float64))
+
+
+def test_kernel_choice_is_a_pure_function_of_the_shape(radlib):
+    """rad_plan_kernel without a device: separable kernel where the grid fills its 16 x 16 x 16 (8) point
+    tiles (BASELINE.json configs 2-5), direct kernel on small angle grids (config 1)."""
+    f = radlib.rad_plan_kernel
+    assert f(256, 32, 32, 0) == 2 and f(512, 64, 64, 2) == 2 and f(128, 16, 16, 0) == 2 and f(1024, 64, 64, 1) == 2
+    assert f(64, 8, 8, 0) == 1 and f(5, 3, 3, 2) == 1
+    radlib.rad_set_kernel(1)
+    assert f(256, 32, 32, 0) == 1
+    radlib.rad_set_kernel(0)
+    with pytest.raises(radlib.RadError):
+        f(0, 4, 4, 0)

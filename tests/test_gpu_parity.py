@@ -424,6 +424,47 @@ def test_sep_ensembles(sep_kernel, oracle_mod, model):
     assert_parity(both, ref, label=f"sep ensemble accumulate model {model}")
 
 
+# ------------------------------------------------------------------ edge cases through the separable kernel too
+def test_sep_straight_line_domain_and_workspace(sep_kernel, oracle_mod):
+    """P1 (zero acceleration -> exactly 0), u >= 1 -> NaN only there, caller workspace == pool scratch,
+    all through the separable kernel (the same checks above run through the direct one)."""
+    import torch
+    rad = sep_kernel
+    wl = workloads.make("cfg2", n=500, n_omega=8, n_th=4)
+    for k in ("ax", "ay", "az"):
+        wl.traj[k] = np.zeros(500)
+    for model in (CL, S0, SH):
+        assert np.all(run_single(rad, wl, model, 1e-16) == 0.0)
+
+    wl = workloads.make("cfg1", n=600, n_omega=8, n_th=2)
+    lam = 1.0000001 / wl.omega[5]
+    cube = run_single(rad, wl, SH, lam)
+    assert np.all(np.isnan(cube[5:])) and np.all(np.isfinite(cube[:5]))
+    assert_parity(cube[:5], oracle_mod.grid(wl.traj, wl.omega[:5], wl.thx, wl.thy, SH, lam), label="sep domain")
+
+    wl = workloads.make("cfg2", n=1500, n_omega=16, n_th=8)
+    tr, g = dev_dict(wl.traj), dev_grid(wl)
+    ws = torch.empty(rad.rad_workspace_bytes(1, 1500, 16, 8, 8), dtype=torch.uint8, device="cuda")
+    a = rad.rad_classical(tr, *g, workspace=ws).cpu().numpy()
+    b = rad.rad_classical(tr, *g).cpu().numpy()
+    assert np.array_equal(a, b)
+
+
+def test_plan_kernel_choice(rad):
+    """rad_plan_kernel: separable where the grid fills its tiles (BASELINE configs 2-5), direct on
+    small angle grids (config 1); rad_set_kernel overrides and is restored."""
+    assert rad.rad_plan_kernel(256, 32, 32, CL) == 2 and rad.rad_plan_kernel(512, 64, 64, SH) == 2
+    assert rad.rad_plan_kernel(128, 16, 16, CL) == 2 and rad.rad_plan_kernel(1024, 64, 64, S0) == 2
+    assert rad.rad_plan_kernel(64, 8, 8, CL) == 1 and rad.rad_plan_kernel(5, 3, 3, SH) == 1
+    rad.rad_set_kernel(1)
+    assert rad.rad_plan_kernel(256, 32, 32, CL) == 1
+    rad.rad_set_kernel(2)
+    assert rad.rad_plan_kernel(5, 3, 3, SH) == 2
+    rad.rad_set_kernel(0)
+    with pytest.raises(rad.RadError):
+        rad.rad_set_kernel(7)
+
+
 def test_sep_matches_direct_kernel(rad, oracle_mod):
     """Both kernels on the same input agree far inside the tolerance (they share only the packed records)."""
     wl = workloads.make("cfg3", n=5000, n_omega=32, n_th=32)
@@ -434,3 +475,41 @@ def test_sep_matches_direct_kernel(rad, oracle_mod):
     rad.rad_set_kernel(0)
     tol = np.maximum(RTOL * np.abs(a), FLOOR * a.max())
     assert np.max(np.abs(a - b) / tol) <= 1.0
+
+
+# ------------------------------------------------------------------ sectioned trajectory (NEXT row N3)
+@pytest.mark.parametrize("kernel", [1, 2])
+def test_sections_sum(rad, oracle_mod, kernel):
+    """one trajectory cut into sections with their own energy; spectrum = sum of the
+    section spectra.  Oracle: the sections copied out as an ensemble (shared boundary samples)."""
+    wl = workloads.make("cfg3", n=3000, n_omega=12, n_th=10, seed=17)
+    start = np.array([0, 700, 701, 1500, 2999], dtype=np.int64)          # one 2-sample section, ragged lengths
+    lam = wl.hbarc_over_E * np.array([1.0, 1.02, 1.05, 1.1])             # energy drops from section to section
+    tr = {k: v.copy() for k, v in wl.traj.items()}
+    for s in range(4):                                                   # per-section gamma, as the paper fixes E per section
+        tr["gamma"][start[s] + (s > 0):start[s + 1] + 1] = wl.meta["gamma"] / (lam[s] / lam[0])
+    nvec = np.diff(start) + 1
+    batch = {k: np.zeros((4, nvec.max())) for k in tr}
+    for s in range(4):
+        for k in tr:
+            batch[k][s, :nvec[s]] = tr[k][start[s]:start[s + 1] + 1]
+    # the shared boundary sample belongs to both neighbours: give it each section's own gamma, as a caller would
+    trs = {k: v.copy() for k, v in tr.items()}
+    w, nx, ny = oracle_mod.grid_points(wl.omega, wl.thx, wl.thy)
+    rad.rad_set_kernel(kernel)
+    try:
+        for model in (CL, SH):
+            ref = oracle_mod.ensemble_points(batch, nvec, w, nx, ny, model, lam if model else None)
+            cube = rad.rad_sections_sum(dev_dict(trs), start, *dev_grid(wl), model=model,
+                                        hbarc_over_E=lam if model else None).cpu().numpy()
+            assert_parity(cube, ref, label=f"sections kernel {kernel} model {model}")
+        half = rad.rad_sections_sum(dev_dict(trs), start[:3], *dev_grid(wl), model=SH, hbarc_over_E=lam[:2])
+        both = rad.rad_sections_sum(dev_dict(trs), start[2:], *dev_grid(wl), model=SH, hbarc_over_E=lam[2:],
+                                    accumulate=True, out=half).cpu().numpy()
+        assert_parity(both, ref, label=f"sections accumulate kernel {kernel}")
+    finally:
+        rad.rad_set_kernel(0)
+    with pytest.raises(rad.RadError):
+        rad.rad_sections_sum(dev_dict(trs), [0, 10, 10], *dev_grid(wl))
+    with pytest.raises(rad.RadError):
+        rad.rad_sections_sum(dev_dict(trs), [0, 3000], *dev_grid(wl))
