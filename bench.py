@@ -35,17 +35,17 @@ sys.path.insert(0, str(ROOT))
 
 METRIC = "fp64_radiation_integral_evals_per_s"
 UNIT = "evals/s"
-# algorithmic FP64 flops per eval, enumerated there operation by operation
-# (phase 2, exact range reduction 3, quarter-angle polynomials 21, two doublings 7, complex
-# accumulation 8 [+4 for spin-1/2's J], integrand geometry 34 [37] per 8 omegas) and checked
-# against ncu's 2*DFMA + DMUL + DADD count (45.6 on cfg2).  SURVEY.md 8(d) estimated 52-60.
+# algorithmic FP64 flops per eval, enumerated there operation by operation.
+# Direct kernel: phase 2, exact range reduction 1 (+ one FRND beside the FP64 pipe), quarter-angle
+# polynomials 21, two doublings 7, complex accumulation 8 [+4 for spin-1/2's J], integrand geometry
+# 34 [37] per 8 omegas -> 43.25 [47.6] flops, 24.6 [26.9] FP64 instructions (SURVEY.md 8(d) estimated 52-60).
 # The separable-phasor kernel needs far fewer: per eval one complex multiply (6) and
 # the accumulation (8 [12]), plus per 16 [8] evals one T and one [half a] Y phasor and one [half an]
-# integrand entry (38 + 37 + 28 [31] flops) -> 20.44 [27.0] flops, 12.0 [15.56] FP64 instructions;
-# ncu counts 11.9 [15.5] instructions per eval.
+# integrand entry (36 + 35 + 28 [31] flops) -> 20.19 [26.63] flops, 11.75 [15.19] FP64 instructions.
+# Both are checked against ncu's 2*DFMA + DMUL + DADD count (profiles/).
 KERNELS = {1: "rad_main_kernel (direct phasor)", 2: "rad_sep_kernel (separable phasor)"}
-FLOPS_PER_EVAL = {1: {0: 45.25, 1: 45.25, 2: 49.6}, 2: {0: 20.44, 1: 20.44, 2: 27.0}}
-FP64_INSTR_PER_EVAL = {1: {0: 26.6, 1: 26.6, 2: 28.9}, 2: {0: 12.0, 1: 12.0, 2: 15.56}}
+FLOPS_PER_EVAL = {1: {0: 43.25, 1: 43.25, 2: 47.6}, 2: {0: 20.19, 1: 20.19, 2: 26.63}}
+FP64_INSTR_PER_EVAL = {1: {0: 24.6, 1: 24.6, 2: 26.9}, 2: {0: 11.75, 1: 11.75, 2: 15.19}}
 FP64_SPEC_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # 148 SM x 64 FMA lanes x 2 x 1.965 GHz
 
 
