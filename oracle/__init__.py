@@ -58,9 +58,49 @@ def build(variant: str = "ld", force: bool = False) -> Path:
     return so
 
 
+def build_traj(force: bool = False) -> Path:
+    """Compile ``traj_oracle.c`` (synthetic-well trajectory generator, long double)."""
+    _BUILD.mkdir(exist_ok=True)
+    so = _BUILD / "libtraj_oracle.so"
+    src = _HERE / "traj_oracle.c"
+    if not force and so.exists() and so.stat().st_mtime >= src.stat().st_mtime:
+        return so
+    tmp = so.with_suffix(f".tmp{os.getpid()}.so")
+    subprocess.run(["gcc", "-std=c11", "-O2", "-fopenmp", "-fPIC", "-shared", "-fno-fast-math",
+                    "-ffp-contract=off", "-o", str(tmp), str(src), "-lm"], check=True)
+    os.replace(tmp, so)
+    return so
+
+
 def build_all() -> None:
     for v in _VARIANTS:
         build(v)
+    build_traj()
+
+
+WELL_COSINE, WELL_AXIAL_EXP = 0, 1
+
+
+def generate(well: int, kappa: float, length: float, gamma: float, dt: float, n: int,
+             x0, y0, vx0, vy0) -> dict:
+    """Oracle trajectories of ``len(x0)`` particles in a synthetic well: FIELDS -> (count, n) arrays."""
+    with _LOCK:
+        if "traj" not in _LIBS:
+            lib = ctypes.CDLL(str(build_traj()))
+            lib.traj_oracle_generate.restype = ctypes.c_int
+            lib.traj_oracle_generate.argtypes = ([ctypes.c_int] + [ctypes.c_double] * 4
+                                                 + [ctypes.c_int32, ctypes.c_int64, ctypes.c_int64]
+                                                 + [_dp] * 15)
+            _LIBS["traj"] = lib
+        lib = _LIBS["traj"]
+    ini = [_f64(a).ravel() for a in (x0, y0, vx0, vy0)]
+    count = ini[0].shape[0]
+    out = {k: np.zeros((count, n)) for k in FIELDS}
+    rc = lib.traj_oracle_generate(int(well), float(kappa), float(length), float(gamma), float(dt), count, n, n,
+                                  *[_ptr(a) for a in ini], *[_ptr(out[k]) for k in FIELDS])
+    if rc != 0:
+        raise ValueError("traj_oracle_generate: invalid arguments")
+    return out
 
 
 def _lib(variant: str) -> ctypes.CDLL:
