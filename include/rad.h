@@ -130,6 +130,27 @@ int rad_sections_sum(const rad_traj *traj, int32_t n_sections, const int64_t *st
 int rad_angular_sum(const double *cube, const rad_grid *grid, double d_solid_angle,
                     double theta_cut, double *spectrum, void *cuda_stream);
 
+/* Trajectories of `count` particles in a static synthetic well, generated on the device in the SoA
+ * layout the calls above read -- the paper's outlook "many particle trajectories evaluated in parallel
+ * on the GPU", for the wells of BASELINE.json configs 3 and 5 (the paper's own solver
+ * needs potential tables that are not available).  Fixed-step velocity Verlet:
+ *   a_k = A(r_k), v_h = v_k + dt/2 a_k, r_{k+1} = r_k + dt v_h, v_{k+1} = v_h + dt/2 A(r_{k+1})
+ *   RAD_WELL_COSINE:     A_x = -kappa sin(2 pi x / length), A_y = 0
+ *   RAD_WELL_AXIAL_EXP:  A = -kappa (r/|r|) exp(-|r| / length), A(0) = 0
+ * and t_k = k dt, dvz = -(vx^2 + vy^2)/2, dz = cumulative trapezoid of dvz (dz_0 = 0),
+ * az = -(vx ax + vy ay) (leading-order relations), gamma_k = gamma.
+ * x0, y0, vx0, vy0: DEVICE arrays of `count` initial values.  out: DEVICE arrays [count][stride], the
+ * first n entries of each row are written (pass them to rad_ensemble_sum as a rad_traj_batch with
+ * the same stride).  One thread per particle: meant for many particles. */
+typedef enum { RAD_WELL_COSINE = 0, RAD_WELL_AXIAL_EXP = 1 } rad_well;
+typedef struct {
+    double *t, *dz, *x, *y, *vx, *vy, *dvz, *ax, *ay, *az, *gamma;
+} rad_traj_buffers;
+int rad_generate_trajectories(rad_well well, double kappa, double length, double gamma, double dt,
+                              int32_t count, int64_t n, int64_t stride,
+                              const double *x0, const double *y0, const double *vx0, const double *vy0,
+                              const rad_traj_buffers *out, void *cuda_stream);
+
 /* out[i] (+)= cubes[0*m + i] + cubes[1*m + i] + ... + cubes[(count-1)*m + i], added in that
  * order (fixed order: deterministic).  Combines the partial cubes of ensemble shards -- other
  * GPUs' (after an all-gather) or successive batches' -- into the ensemble sum of PAPER.md:75,

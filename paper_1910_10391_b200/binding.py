@@ -19,7 +19,8 @@ FIELDS = ("t", "dz", "x", "y", "vx", "vy", "dvz", "ax", "ay", "az", "gamma")
 EXPORTS = ("rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_sections_sum", "rad_angular_sum", "rad_sum_cubes",
            "rad_workspace_bytes", "rad_eval_host", "rad_ensemble_sum_host",
            "rad_measure_fp64_peak", "rad_launch_count", "rad_strerror",
-           "rad_profile_enable", "rad_profile_last", "rad_set_kernel", "rad_plan_kernel")
+           "rad_profile_enable", "rad_profile_last", "rad_set_kernel", "rad_plan_kernel",
+           "rad_generate_trajectories")
 
 _dp = ctypes.POINTER(ctypes.c_double)
 _lib = None
@@ -52,7 +53,8 @@ def library_path() -> Path:
 def build_library(force: bool = False, verbose: bool = False) -> Path:
     """Compile csrc/rad.cu for sm_100a into the in-tree shared library (nvcc cross-compiles
     without a GPU)."""
-    srcs = [_SRC / "rad.cu", _SRC / "rad_device.cuh", _SRC / "rad_sep.cuh", _SRC / "sincos_coeffs.h",
+    srcs = [_SRC / "rad.cu", _SRC / "rad_device.cuh", _SRC / "rad_sep.cuh", _SRC / "rad_traj.cuh",
+            _SRC / "sincos_coeffs.h",
             _PKG.parent / "include" / "rad.h"]
     if not force and _SO.exists() and all(_SO.stat().st_mtime >= s.stat().st_mtime for s in srcs):
         return _SO
@@ -241,6 +243,39 @@ def rad_angular_sum(cube, omega, thx, thy, d_solid_angle: float, theta_cut: floa
         out = torch.empty(omega.numel(), dtype=torch.float64, device=cube.device)
     _check(load_library().rad_angular_sum(cube.data_ptr(), ctypes.byref(g), float(d_solid_angle),
                                           float(theta_cut), _dev(out, "out").data_ptr(), _stream_ptr(stream)))
+    return out
+
+
+WELL_COSINE, WELL_AXIAL_EXP = 0, 1
+
+
+class _TrajBuffers(ctypes.Structure):
+    _fields_ = [(k, ctypes.c_void_p) for k in FIELDS]
+
+
+def rad_generate_trajectories(well: int, kappa: float, length: float, gamma: float, dt: float, n: int,
+                              x0, y0, vx0, vy0, out: dict | None = None, stream=None) -> dict:
+    """`count` particles in a synthetic well, generated on the device (PAPER.md:233 outlook): FIELDS ->
+    (count, n) CUDA tensors ready for rad_ensemble_sum."""
+    ini = [_dev(a, name) for a, name in ((x0, "x0"), (y0, "y0"), (vx0, "vx0"), (vy0, "vy0"))]
+    count = ini[0].numel()
+    if any(a.numel() != count for a in ini):
+        raise ValueError("x0, y0, vx0, vy0 must have one length")
+    if out is None:
+        out = {k: torch.empty((count, n), dtype=torch.float64, device=ini[0].device) for k in FIELDS}
+    ts = [_dev(out[k], k) for k in FIELDS]
+    stride = ts[0].shape[1]
+    if any(tuple(t.shape) != (count, stride) for t in ts):
+        raise ValueError("out tensors must share one (count, stride) shape")
+    bufs = _TrajBuffers(*[t.data_ptr() for t in ts])
+    lib = load_library()
+    lib.rad_generate_trajectories.argtypes = ([ctypes.c_int] + [ctypes.c_double] * 4
+                                              + [ctypes.c_int32, ctypes.c_int64, ctypes.c_int64]
+                                              + [ctypes.c_void_p] * 4 + [ctypes.POINTER(_TrajBuffers), ctypes.c_void_p])
+    lib.rad_generate_trajectories.restype = ctypes.c_int
+    _check(lib.rad_generate_trajectories(int(well), float(kappa), float(length), float(gamma), float(dt), count,
+                                         int(n), int(stride), *[a.data_ptr() for a in ini], ctypes.byref(bufs),
+                                         _stream_ptr(stream)))
     return out
 
 

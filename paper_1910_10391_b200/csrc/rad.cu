@@ -60,6 +60,7 @@ struct MainParams {
 
 }  // namespace rad
 #include "rad_sep.cuh"
+#include "rad_traj.cuh"
 namespace rad {
 
 // ------------------------------------------------------------------------------ pack (a0, a1)
@@ -766,6 +767,29 @@ int rad_angular_sum(const double *cube, const rad_grid *grid, double d_solid_ang
     rad_angular_sum_kernel<<<grid->n_omega, 256, 0, st>>>(
         cube, grid->thx, grid->thy, grid->n_thx, grid->n_thy, d_solid_angle,
         theta_cut > 0.0 ? theta_cut * theta_cut : 0.0, spectrum);
+    ++g_launches;
+    CK(cudaGetLastError());
+    return RAD_OK;
+}
+
+int rad_generate_trajectories(rad_well well, double kappa, double length, double gamma, double dt,
+                              int32_t count, int64_t n, int64_t stride,
+                              const double *x0, const double *y0, const double *vx0, const double *vy0,
+                              const rad_traj_buffers *out, void *cuda_stream) {
+    if (!out || !x0 || !y0 || !vx0 || !vy0 || count < 1 || n < 2 || stride < n) return RAD_EINVAL;
+    if (well != RAD_WELL_COSINE && well != RAD_WELL_AXIAL_EXP) return RAD_EINVAL;
+    if (!(dt > 0.0) || !(length > 0.0) || !(gamma >= 1.0)) return RAD_EDOMAIN;
+    double *arrs[11] = {out->t, out->dz, out->x, out->y, out->vx, out->vy, out->dvz, out->ax, out->ay, out->az,
+                        out->gamma};
+    for (double *p : arrs)
+        if (!p || !aligned8(p)) return RAD_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const TrajOut o{out->t, out->dz, out->x, out->y, out->vx, out->vy, out->dvz, out->ax, out->ay, out->az, out->gamma};
+    const unsigned blocks = (unsigned)((count + 127) / 128);
+    if (well == RAD_WELL_COSINE)
+        rad_traj_kernel<0><<<blocks, 128, 0, st>>>(kappa, length, gamma, dt, count, n, stride, x0, y0, vx0, vy0, o);
+    else
+        rad_traj_kernel<1><<<blocks, 128, 0, st>>>(kappa, length, gamma, dt, count, n, stride, x0, y0, vx0, vy0, o);
     ++g_launches;
     CK(cudaGetLastError());
     return RAD_OK;
