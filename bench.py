@@ -46,6 +46,10 @@ UNIT = "evals/s"
 KERNELS = {1: "rad_main_kernel (direct phasor)", 2: "rad_sep_kernel (separable phasor)"}
 FLOPS_PER_EVAL = {1: {0: 43.25, 1: 43.25, 2: 47.6}, 2: {0: 20.19, 1: 20.19, 2: 26.63}}
 FP64_INSTR_PER_EVAL = {1: {0: 24.6, 1: 24.6, 2: 26.9}, 2: {0: 11.75, 1: 11.75, 2: 15.19}}
+# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the main kernel, from the ncu --set full
+# captures under profiles/ (r01_*_ncu_full.txt); bench.py cannot run ncu itself, other workloads report null.
+NCU_TRAFFIC_BYTES = {("cfg2", 2): 1.256704e6 + 75.79136e6, ("cfg2", 1): 1.2224e6 + 8.14976e6,
+                     ("cfg3", 2): 16.3904e6 + 10496.0, ("cfg3", 1): 16.240128e6 + 6144.0}
 FP64_SPEC_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # 148 SM x 64 FMA lanes x 2 x 1.965 GHz
 
 
@@ -352,7 +356,9 @@ def run_b200(args):
             "gpu_launches": int(launches),
             "roofline": {"bound": "alu", "kernel": KERNELS[kernel],
                          "achieved": achieved / 1e12, "peak": peak / 1e12, "unit": "TFLOP/s",
-                         "frac": achieved / peak, "traffic": None,
+                         "frac": achieved / peak,
+                         "traffic": NCU_TRAFFIC_BYTES.get((args.workload, kernel)) if args.spin == "1/2" else None,
+                         "traffic_unit": "bytes per main-kernel launch (ncu capture in profiles/, not this run)",
                          "peak_kind": "FP64 FMA microbenchmark measured in this run (rad_measure_fp64_peak)",
                          "peak_spec": FP64_SPEC_TFLOPS, "frac_of_spec": achieved / 1e12 / FP64_SPEC_TFLOPS,
                          "flops_per_eval": FLOPS_PER_EVAL[kernel][model],

@@ -513,3 +513,28 @@ def test_sections_sum(rad, oracle_mod, kernel):
         rad.rad_sections_sum(dev_dict(trs), [0, 10, 10], *dev_grid(wl))
     with pytest.raises(rad.RadError):
         rad.rad_sections_sum(dev_dict(trs), [0, 3000], *dev_grid(wl))
+
+
+# ------------------------------------------------------------------ extreme shapes the paper names
+def test_three_thousand_squared_angles(rad, oracle_mod):
+    """"more than 3000^2" angular points without multiple scattering.  2 omegas x 3000 x 3000
+    angles = 1.8e7 integrals (144 MB cube) over a short trajectory; sampled against the oracle."""
+    wl = workloads.make("cfg2", n=150, n_omega=2, n_th=3000, seed=33)
+    cube = run_single(rad, wl, CL, 0.0)
+    assert cube.shape == (2, 3000, 3000)
+    idx, ref = sampled_reference(oracle_mod, wl, cube, 4000, (2, 7, 7), CL, 0.0)
+    assert_parity(cube, ref, idx, label="3000^2 angles")
+
+
+@pytest.mark.parametrize("kernel", [1, 2])
+def test_million_samples_on_a_small_grid(rad, oracle_mod, kernel):
+    """configs[4]'s trajectory length (N = 1e6, phases to 3.8e6 rad) on a grid small enough that the time
+    axis is split across the whole GPU (7813 chunks), both kernels, spin-1/2."""
+    wl = workloads.make("cfg5", n=1000000, n_omega=16, n_th=16)
+    rad.rad_set_kernel(kernel)
+    try:
+        cube = run_single(rad, wl, SH, wl.hbarc_over_E)
+    finally:
+        rad.rad_set_kernel(0)
+    idx, ref = sampled_reference(oracle_mod, wl, cube, 40, (3, 3, 3), SH, wl.hbarc_over_E)
+    assert_parity(cube, ref, idx, label=f"N=1e6 kernel {kernel}")
