@@ -41,6 +41,10 @@ class _Batch(ctypes.Structure):
                 + [(k, ctypes.c_void_p) for k in FIELDS])
 
 
+class _TrajBuffers(ctypes.Structure):
+    _fields_ = [(k, ctypes.c_void_p) for k in FIELDS]
+
+
 class _Grid(ctypes.Structure):
     _fields_ = [("n_omega", ctypes.c_int32), ("n_thx", ctypes.c_int32), ("n_thy", ctypes.c_int32),
                 ("omega", ctypes.c_void_p), ("thx", ctypes.c_void_p), ("thy", ctypes.c_void_p)]
@@ -88,6 +92,13 @@ def load_library() -> ctypes.CDLL:
     lib.rad_sections_sum.restype = ctypes.c_int
     lib.rad_angular_sum.argtypes = [vp, ctypes.POINTER(_Grid), dbl, dbl, vp, vp]
     lib.rad_sum_cubes.argtypes = [vp, i32, i64, ctypes.c_int, vp, vp]
+    lib.rad_set_kernel.argtypes = [ctypes.c_int]
+    lib.rad_set_kernel.restype = ctypes.c_int
+    lib.rad_plan_kernel.argtypes = [i32, i32, i32, ctypes.c_int]
+    lib.rad_plan_kernel.restype = ctypes.c_int
+    lib.rad_generate_trajectories.argtypes = ([ctypes.c_int] + [dbl] * 4 + [i32, i64, i64] + [vp] * 4
+                                              + [ctypes.POINTER(_TrajBuffers), vp])
+    lib.rad_generate_trajectories.restype = ctypes.c_int
     lib.rad_workspace_bytes.argtypes = [i32, i64, i32, i32, i32]
     lib.rad_workspace_bytes.restype = sz
     lib.rad_eval_host.argtypes = [ctypes.POINTER(_Traj), ctypes.POINTER(_Grid), ctypes.c_int, dbl, vp, vp]
@@ -249,10 +260,6 @@ def rad_angular_sum(cube, omega, thx, thy, d_solid_angle: float, theta_cut: floa
 WELL_COSINE, WELL_AXIAL_EXP = 0, 1
 
 
-class _TrajBuffers(ctypes.Structure):
-    _fields_ = [(k, ctypes.c_void_p) for k in FIELDS]
-
-
 def rad_generate_trajectories(well: int, kappa: float, length: float, gamma: float, dt: float, n: int,
                               x0, y0, vx0, vy0, out: dict | None = None, stream=None) -> dict:
     """`count` particles in a synthetic well, generated on the device (PAPER.md:233 outlook): FIELDS ->
@@ -268,12 +275,7 @@ def rad_generate_trajectories(well: int, kappa: float, length: float, gamma: flo
     if any(tuple(t.shape) != (count, stride) for t in ts):
         raise ValueError("out tensors must share one (count, stride) shape")
     bufs = _TrajBuffers(*[t.data_ptr() for t in ts])
-    lib = load_library()
-    lib.rad_generate_trajectories.argtypes = ([ctypes.c_int] + [ctypes.c_double] * 4
-                                              + [ctypes.c_int32, ctypes.c_int64, ctypes.c_int64]
-                                              + [ctypes.c_void_p] * 4 + [ctypes.POINTER(_TrajBuffers), ctypes.c_void_p])
-    lib.rad_generate_trajectories.restype = ctypes.c_int
-    _check(lib.rad_generate_trajectories(int(well), float(kappa), float(length), float(gamma), float(dt), count,
+    _check(load_library().rad_generate_trajectories(int(well), float(kappa), float(length), float(gamma), float(dt), count,
                                          int(n), int(stride), *[a.data_ptr() for a in ini], ctypes.byref(bufs),
                                          _stream_ptr(stream)))
     return out
@@ -357,18 +359,12 @@ def rad_launch_count() -> int:
 
 def rad_set_kernel(choice: int = 0) -> None:
     """0: choose by grid shape (default), 1: direct-phasor kernel, 2: separable-phasor kernel."""
-    lib = load_library()
-    lib.rad_set_kernel.argtypes = [ctypes.c_int]
-    lib.rad_set_kernel.restype = ctypes.c_int
-    _check(lib.rad_set_kernel(int(choice)))
+    _check(load_library().rad_set_kernel(int(choice)))
 
 
 def rad_plan_kernel(n_omega: int, n_thx: int, n_thy: int, model: int = CLASSICAL) -> int:
     """1: direct-phasor kernel, 2: separable-phasor kernel, for a grid of this shape (current setting)."""
-    lib = load_library()
-    lib.rad_plan_kernel.argtypes = [ctypes.c_int32, ctypes.c_int32, ctypes.c_int32, ctypes.c_int]
-    lib.rad_plan_kernel.restype = ctypes.c_int
-    rc = lib.rad_plan_kernel(n_omega, n_thx, n_thy, int(model))
+    rc = load_library().rad_plan_kernel(n_omega, n_thx, n_thy, int(model))
     if rc < 0:
         _check(rc)
     return rc

@@ -12,6 +12,10 @@
 //   rad_finalize_kernel  a6/a7  ordered reduction of time-split amplitudes / trajectory-split
 //                               spectra
 //   rad_angular_sum_kernel      sum of the cube over angles
+//   rad_sep_kernel (rad_sep.cuh) a0-a7 again for tensor grids that fill its tiles: the phasor of eq. (7)
+//                               factorised into T(omega, n_x) Y(omega, n_y), warp-specialised CTA
+//   rad_sum_cubes_kernel        ordered sum of partial cubes (ensemble shards)
+//   rad_traj_kernel (rad_traj.cuh)  synthetic-well trajectories on the device
 #include <atomic>
 #include <cmath>
 #include <cstdio>
@@ -28,9 +32,6 @@ namespace rad {
 
 #ifndef RAD_W
 #define RAD_W 8
-#endif
-#ifndef RAD_MINB
-#define RAD_MINB 1
 #endif
 #ifndef RAD_DEG
 #define RAD_DEG 5            // polynomial set of sincos_coeffs.h: 5 = LO (1e-13, default), 6 = HI (2e-16)
@@ -146,7 +147,7 @@ __device__ __forceinline__ double spectrum_value(const double (&acc)[NC], double
 // ------------------------------------------------------------------------------ main (a0-a5)
 // NC = number of real accumulators per omega: 4 (A_x, A_y) or 6 (+ J, spin-1/2).
 template <int NC, int DEG>
-__global__ void __launch_bounds__(TPB, RAD_MINB)
+__global__ void __launch_bounds__(TPB, 1)
 rad_main_kernel(const MainParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
     double *ring = reinterpret_cast<double *>(smem_raw);
@@ -348,9 +349,10 @@ rad_finalize_kernel(const MainParams P) {
     if (gid >= T) return;
     const int wg = (int)(gid / A), a = (int)(gid % A);
     const double nx = P.thx[a % P.n_thx], ny = P.thy[a / P.n_thx];
-    for (int j = 0; j < W; ++j) {
+    {                                                 // gridDim.y = W: one omega of the register tile per CTA row
+        const int j = blockIdx.y;
         const int iw = wg * W + j;
-        if (iw >= P.n_omega) break;
+        if (iw >= P.n_omega) return;
         const double om = P.omega[iw];
         double total = 0.0;
         if (P.mode == MODE_PSLICE) {
@@ -512,7 +514,7 @@ static Plan make_plan(int count, int64_t n_max, int n_omega, int n_thx, int n_th
         // waves of 2 * sms to >= 98.5 %
         const int slots = 2 * sms;
         if (pl.tiles < 8 * sms) {
-            const int64_t kmax = std::max<int64_t>(1, (int64_t)count * std::max(1, pl.cpt / 2));
+            const int64_t kmax = std::max<int64_t>(1, (int64_t)count * std::max(1, pl.cpt));
             int best_k = 1;
             double best = 0.0;
             for (int64_t k = 1; k <= std::min<int64_t>(kmax, 8 * sms); ++k) {
@@ -525,7 +527,7 @@ static Plan make_plan(int count, int64_t n_max, int n_omega, int n_thx, int n_th
             if (best_k > 1) {
                 if (count >= best_k) { pl.mode = MODE_PSLICE; pl.p_slices = best_k; }
                 else {
-                    int ts = std::min((best_k + count - 1) / count, std::max(1, pl.cpt / 2));
+                    int ts = std::min((best_k + count - 1) / count, std::max(1, pl.cpt));
                     if (ts > 1) { pl.mode = MODE_TSPLIT; pl.t_slices = ts; pl.p_slices = count; }
                     else if (count > 1) { pl.mode = MODE_PSLICE; pl.p_slices = count; }
                 }
@@ -695,8 +697,8 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const int64
             if (nc == 6) rad_sep_finalize_kernel<6, 2><<<dim3(pl.tiles, 8), SEP_CONS, 0, st>>>(mp);
             else rad_sep_finalize_kernel<4, 4><<<dim3(pl.tiles, 16), SEP_CONS, 0, st>>>(mp);
         } else {
-            if (nc == 6) rad_finalize_kernel<6><<<pl.tiles, TPB, 0, st>>>(mp);
-            else rad_finalize_kernel<4><<<pl.tiles, TPB, 0, st>>>(mp);
+            if (nc == 6) rad_finalize_kernel<6><<<dim3(pl.tiles, W), TPB, 0, st>>>(mp);
+            else rad_finalize_kernel<4><<<dim3(pl.tiles, W), TPB, 0, st>>>(mp);
         }
         ++g_launches;
         CK(cudaGetLastError());

@@ -113,14 +113,6 @@ __device__ __forceinline__ void sincos_poly<5>(double z, double &ps, double &pc)
 #pragma unroll
     for (int i = 4; i >= 0; --i) { ps = fma(ps, z, SC_S5[i]); pc = fma(pc, z, SC_C5[i]); }
 }
-// sine of set 5 (4.7e-15) with cosine of set 6 (2e-16): one DFMA less than <6>
-template <>
-__device__ __forceinline__ void sincos_poly<56>(double z, double &ps, double &pc) {
-    ps = SC_S5[5]; pc = fma(SC_C6[6], z, SC_C6[5]);
-#pragma unroll
-    for (int i = 4; i >= 0; --i) { ps = fma(ps, z, SC_S5[i]); pc = fma(pc, z, SC_C6[i]); }
-}
-
 template <int DEG>
 __device__ __forceinline__ void phasor_turns(double p, double &c_out, double &s_out) {
 #ifndef RAD_MAGIC_REDUCTION

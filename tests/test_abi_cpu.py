@@ -37,7 +37,8 @@ def test_library_is_sm100a_with_tma(radlib):
                           text=True, check=True).stdout
     assert "sm_100a" in sass
     assert "UBLKCP" in sass and "SYNCS" in sass
-    assert "DFMA" in sass
+    assert "DFMA" in sass and "FRND.F64" in sass
+    assert "USETMAXREG" in sass                      # the separable kernel's producer / consumer register split
 
 
 def test_strerror_and_launch_count(radlib):
