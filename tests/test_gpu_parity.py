@@ -538,3 +538,26 @@ def test_million_samples_on_a_small_grid(rad, oracle_mod, kernel):
         rad.rad_set_kernel(0)
     idx, ref = sampled_reference(oracle_mod, wl, cube, 40, (3, 3, 3), SH, wl.hbarc_over_E)
     assert_parity(cube, ref, idx, label=f"N=1e6 kernel {kernel}")
+
+
+# ------------------------------------------------------------------ configs[3] and configs[4] at FULL size
+@pytest.mark.parametrize("model", [S0, SH])
+def test_cfg5_full_size_sampled(rad, oracle_mod, model):
+    """BASELINE.json configs[4] exactly (N = 1e6, 1024 x 64 x 64, phases to 3.8e6 rad), both spin variants,
+    in the launch configuration bench.py times (the library's own kernel choice); sampled outputs."""
+    wl = workloads.make("cfg5", model=model)
+    cube = run_single(rad, wl, model, wl.hbarc_over_E)
+    idx, ref = sampled_reference(oracle_mod, wl, cube, 48, (3, 3, 3), model, wl.hbarc_over_E)
+    assert_parity(cube, ref, idx, label=f"cfg5 FULL model {model}")
+
+
+def test_cfg4_full_size_sampled(rad, oracle_mod):
+    """BASELINE.json configs[3] exactly: 1000 trajectories x 1e5 samples (8.8 GB of trajectories) summed on the
+    128 x 16 x 16 grid, as bench.py --workload cfg4 times it; a dozen sampled points (1e8 samples each)."""
+    we = workloads.make("cfg4")
+    cube = rad.rad_ensemble_sum(dev_dict(we.batch), we.n, *dev_grid(we)).cpu().numpy()
+    idx = workloads.sample_points(we, 10, (0, 0, 0))
+    idx = np.unique(np.concatenate([idx, [int(np.argmax(cube))]]))
+    w, nx, ny = workloads.points_of(we, idx)
+    ref = oracle_mod.ensemble_points(we.batch, we.n, w, nx, ny)
+    assert_parity(cube, ref, idx, label="cfg4 FULL")
