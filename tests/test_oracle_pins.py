@@ -353,3 +353,48 @@ def test_grid_order(oracle_mod):
     assert cube.shape == (3, 2, 4)
     one = oracle_mod.points(wl.traj, [wl.omega[2]], [wl.thx[3]], [wl.thy[1]])[0]
     assert cube[2, 1, 3] == one
+
+
+# --------------------------------------------------------------------------- symmetries of eq. (1)
+def _sym_workload():
+    import workloads
+    wl = workloads.make("cfg5", n=1500, n_omega=5, n_th=4, seed=9)
+    rng = np.random.Generator(np.random.PCG64(4))
+    nx = rng.uniform(-5e-5, 5e-5, 12)
+    ny = rng.uniform(-5e-5, 5e-5, 12)
+    om = np.repeat(wl.omega[1:4], 4)
+    return wl, om, nx, ny
+
+
+@pytest.mark.parametrize("model", [0, 2])
+def test_translation_and_time_shift_invariance(oracle_mod, model):
+    """A constant shift of x, y or of the time origin multiplies every amplitude of eq. (1) by one common
+    phase factor: the spectrum does not change (catches a wrong sign or coefficient in eq. 7)."""
+    wl, om, nx, ny = _sym_workload()
+    lam = wl.hbarc_over_E
+    base = oracle_mod.points(wl.traj, om, nx, ny, model, lam)
+    tr = {k: v.copy() for k, v in wl.traj.items()}
+    tr["x"] += 3e-10
+    tr["y"] -= 1e-10
+    np.testing.assert_allclose(oracle_mod.points(tr, om, nx, ny, model, lam), base, rtol=2e-9)
+    tr = {k: v.copy() for k, v in wl.traj.items()}
+    tr["t"] += 2.5e-7
+    np.testing.assert_allclose(oracle_mod.points(tr, om, nx, ny, model, lam), base, rtol=2e-9)
+
+
+@pytest.mark.parametrize("model", [0, 2])
+def test_mirror_and_axis_swap_symmetry(oracle_mod, model):
+    """Mirroring the trajectory in x (x, vx, ax -> -x, -vx, -ax) maps the spectrum at n_x to the one at
+    -n_x; exchanging the roles of x and y maps (n_x, n_y) to (n_y, n_x).  The second one pins eq. (4)
+    against eq. (3): they must be each other's image under x <-> y."""
+    wl, om, nx, ny = _sym_workload()
+    lam = wl.hbarc_over_E
+    base = oracle_mod.points(wl.traj, om, nx, ny, model, lam)
+    tr = {k: v.copy() for k, v in wl.traj.items()}
+    for k in ("x", "vx", "ax"):
+        tr[k] = -tr[k]
+    np.testing.assert_allclose(oracle_mod.points(tr, om, -nx, ny, model, lam), base, rtol=1e-12)
+    tr = {k: v.copy() for k, v in wl.traj.items()}
+    for a, b in (("x", "y"), ("vx", "vy"), ("ax", "ay")):
+        tr[a], tr[b] = wl.traj[b].copy(), wl.traj[a].copy()
+    np.testing.assert_allclose(oracle_mod.points(tr, om, ny, nx, model, lam), base, rtol=1e-12)
