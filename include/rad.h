@@ -192,6 +192,14 @@ int rad_set_kernel(int choice);
  * 1 direct, 2 separable (a pure function of the arguments; no device needed); RAD_EINVAL on bad input. */
 int rad_plan_kernel(int32_t n_omega, int32_t n_thx, int32_t n_thy, rad_model model);
 
+/* The launch plan of a call of this shape (a pure function of the arguments, the rad_set_kernel setting and
+ * the SM count; 148 SMs assumed when no device is visible): plan[0] kernel (1 direct, 2 separable),
+ * plan[1] mode (0 one CTA per tile, 1 trajectory axis sliced, 2 time axis sliced), plan[2] tiles =
+ * gridDim.x, plan[3] slices = gridDim.y, plan[4] time slices per trajectory, plan[5] chunks of 128
+ * samples per trajectory.  For inspection and tests. */
+int rad_plan_describe(int32_t count, int64_t n_max, int32_t n_omega, int32_t n_thx, int32_t n_thy,
+                      rad_model model, int32_t *plan);
+
 /* Per-kernel timing of the most recent device-buffer call (for the roofline in bench.py).
  * rad_profile_enable(1) makes every later call record CUDA events on its stream around the
  * pack, main and finalize kernels; rad_profile_last waits for that call's last event and

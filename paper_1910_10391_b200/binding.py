@@ -20,7 +20,7 @@ EXPORTS = ("rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_sectio
            "rad_workspace_bytes", "rad_eval_host", "rad_ensemble_sum_host",
            "rad_measure_fp64_peak", "rad_launch_count", "rad_strerror",
            "rad_profile_enable", "rad_profile_last", "rad_set_kernel", "rad_plan_kernel",
-           "rad_generate_trajectories")
+           "rad_generate_trajectories", "rad_plan_describe")
 
 _dp = ctypes.POINTER(ctypes.c_double)
 _lib = None
@@ -96,6 +96,8 @@ def load_library() -> ctypes.CDLL:
     lib.rad_set_kernel.restype = ctypes.c_int
     lib.rad_plan_kernel.argtypes = [i32, i32, i32, ctypes.c_int]
     lib.rad_plan_kernel.restype = ctypes.c_int
+    lib.rad_plan_describe.argtypes = [i32, i64, i32, i32, i32, ctypes.c_int, ctypes.POINTER(ctypes.c_int32)]
+    lib.rad_plan_describe.restype = ctypes.c_int
     lib.rad_generate_trajectories.argtypes = ([ctypes.c_int] + [dbl] * 4 + [i32, i64, i64] + [vp] * 4
                                               + [ctypes.POINTER(_TrajBuffers), vp])
     lib.rad_generate_trajectories.restype = ctypes.c_int
@@ -368,6 +370,14 @@ def rad_plan_kernel(n_omega: int, n_thx: int, n_thy: int, model: int = CLASSICAL
     if rc < 0:
         _check(rc)
     return rc
+
+
+def rad_plan_describe(count: int, n_max: int, n_omega: int, n_thx: int, n_thy: int, model: int = CLASSICAL) -> dict:
+    """Launch plan of a call of this shape: kernel (1 direct, 2 separable), mode (0 direct, 1 trajectory
+    slices, 2 time slices), tiles (gridDim.x), slices (gridDim.y), t_slices, chunks per trajectory."""
+    plan = (ctypes.c_int32 * 6)()
+    _check(load_library().rad_plan_describe(count, n_max, n_omega, n_thx, n_thy, int(model), plan))
+    return dict(zip(("kernel", "mode", "tiles", "slices", "t_slices", "chunks"), (int(v) for v in plan)))
 
 
 def rad_profile_enable(on: bool = True) -> None:

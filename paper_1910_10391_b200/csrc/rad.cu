@@ -901,6 +901,21 @@ int rad_plan_kernel(int32_t n_omega, int32_t n_thx, int32_t n_thy, rad_model mod
     return choose_kernel(n_omega, n_thx, n_thy, model == RAD_SPIN_HALF ? 6 : 4) + 1;
 }
 
+int rad_plan_describe(int32_t count, int64_t n_max, int32_t n_omega, int32_t n_thx, int32_t n_thy, rad_model model,
+                      int32_t *plan) {
+    if (!plan || count < 1 || n_max < 2 || n_omega < 1 || n_thx < 1 || n_thy < 1) return RAD_EINVAL;
+    if (model < RAD_CLASSICAL || model > RAD_SPIN_HALF) return RAD_EINVAL;
+    const int nc = model == RAD_SPIN_HALF ? 6 : 4;
+    const Plan pl = make_plan(count, n_max, n_omega, n_thx, n_thy, nc, choose_kernel(n_omega, n_thx, n_thy, nc));
+    plan[0] = pl.kernel + 1;
+    plan[1] = pl.mode;
+    plan[2] = pl.tiles;
+    plan[3] = pl.mode == MODE_TSPLIT ? count * pl.t_slices : pl.p_slices;      // gridDim.y
+    plan[4] = pl.t_slices;
+    plan[5] = pl.cpt;
+    return RAD_OK;
+}
+
 int rad_set_kernel(int choice) {
     if (choice < 0 || choice > 2) return RAD_EINVAL;
     g_kernel_choice.store(choice);

@@ -123,3 +123,35 @@ def test_kernel_choice_is_a_pure_function_of_the_shape(radlib):
     radlib.rad_set_kernel(0)
     with pytest.raises(radlib.RadError):
         f(0, 4, 4, 0)
+
+
+def test_launch_plans_of_the_baseline_configs(radlib):
+    """The plan is host logic: a pure function of the shapes (148 SMs assumed without a device).  The five
+    BASELINE.json configs get whole waves of CTAs: separable kernel 1 CTA/SM, direct kernel 2 CTAs/SM."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("plan depends on the visible device's SM count; this checks the 148-SM default")
+    d = radlib.rad_plan_describe
+    p = d(1, 4000, 64, 8, 8, 0)                      # cfg 1: direct kernel, 4 tiles x 32 one-chunk time slices
+    assert (p["kernel"], p["mode"], p["tiles"], p["slices"], p["chunks"]) == (1, 2, 4, 32, 32)
+    p = d(1, 14287, 256, 32, 32, 0)                  # cfg 2: 64 tiles x 16 time slices = 6.92 waves of 148
+    assert (p["kernel"], p["mode"], p["tiles"], p["slices"]) == (2, 2, 64, 16)
+    p = d(1, 200000, 512, 64, 64, 2)                 # cfg 3 spin-1/2: 16 x 16 x 8 point tiles -> 1024 CTAs = 6.92 waves
+    assert (p["kernel"], p["mode"], p["tiles"], p["slices"]) == (2, 0, 1024, 1)
+    p = d(1, 200000, 512, 64, 64, 1)                 # cfg 3 spin-0: 16 x 16 x 16 tiles -> 512 tiles x 2 time slices
+    assert (p["kernel"], p["mode"], p["tiles"], p["slices"]) == (2, 2, 512, 2)
+    p = d(1000, 100000, 128, 16, 16, 0)              # cfg 4: 8 tiles x 37 trajectory slices = 2 waves
+    assert (p["kernel"], p["mode"], p["tiles"], p["slices"]) == (2, 1, 8, 37)
+    p = d(1, 1000000, 1024, 64, 64, 1)               # cfg 5 spin-0: 1024 tiles, one CTA per tile
+    assert (p["kernel"], p["mode"], p["tiles"], p["slices"]) == (2, 0, 1024, 1)
+    p = d(1, 1000000, 1024, 64, 64, 2)               # cfg 5 spin-1/2: 2048 tiles = 13.8 waves
+    assert (p["kernel"], p["mode"], p["tiles"], p["slices"]) == (2, 0, 2048, 1)
+    radlib.rad_set_kernel(1)
+    try:
+        p = d(1, 14287, 256, 32, 32, 0)              # direct kernel on cfg 2: 256 tiles x 8 = 6.92 waves of 296
+        assert (p["kernel"], p["mode"], p["tiles"], p["slices"]) == (1, 2, 256, 8)
+    finally:
+        radlib.rad_set_kernel(0)
+    for k in range(1, 60):                           # slices never exceed the work there is
+        p = d(k, 300, 16, 16, 16, 0)
+        assert p["slices"] <= k * p["chunks"] and p["slices"] >= 1
