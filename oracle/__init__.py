@@ -78,25 +78,53 @@ def build_all() -> None:
     build_traj()
 
 
-WELL_COSINE, WELL_AXIAL_EXP = 0, 1
+WELL_COSINE, WELL_AXIAL_EXP, WELL_HARMONIC_MS = 0, 1, 2
+
+
+def _traj_lib():
+    generate(0, 0.0, 1.0, 1.0, 1.0, 2, [0.0], [0.0], [0.0], [0.0])       # builds and loads on first use
+    return _LIBS["traj"]
+
+
+def philox4x32_10(counter, key):
+    """Philox4x32-10 block (for the known-answer pin): 4 + 2 uint32 in, 4 uint32 out."""
+    c = np.ascontiguousarray(counter, dtype=np.uint32)
+    k = np.ascontiguousarray(key, dtype=np.uint32)
+    out = np.zeros(4, dtype=np.uint32)
+    u32p = ctypes.POINTER(ctypes.c_uint32)
+    _traj_lib().traj_oracle_philox(c.ctypes.data_as(u32p), k.ctypes.data_as(u32p), out.ctypes.data_as(u32p))
+    return out
+
+
+def kick_normals(seed: int, particle: int, n: int):
+    """The standard normals (xi1, xi2) of steps 0..n-1 of one particle of the scattering well."""
+    a, b = np.zeros(n), np.zeros(n)
+    _traj_lib().traj_oracle_normals(int(seed), int(particle), int(n), _ptr(a), _ptr(b))
+    return a, b
 
 
 def generate(well: int, kappa: float, length: float, gamma: float, dt: float, n: int,
-             x0, y0, vx0, vy0) -> dict:
+             x0, y0, vx0, vy0, sigma: float = 0.0, seed: int = 0) -> dict:
     """Oracle trajectories of ``len(x0)`` particles in a synthetic well: FIELDS -> (count, n) arrays."""
     with _LOCK:
         if "traj" not in _LIBS:
             lib = ctypes.CDLL(str(build_traj()))
             lib.traj_oracle_generate.restype = ctypes.c_int
-            lib.traj_oracle_generate.argtypes = ([ctypes.c_int] + [ctypes.c_double] * 4
+            lib.traj_oracle_generate.argtypes = ([ctypes.c_int] + [ctypes.c_double] * 5 + [ctypes.c_uint64]
                                                  + [ctypes.c_int32, ctypes.c_int64, ctypes.c_int64]
                                                  + [_dp] * 15)
+            u32p = ctypes.POINTER(ctypes.c_uint32)
+            lib.traj_oracle_philox.argtypes = [u32p, u32p, u32p]
+            lib.traj_oracle_philox.restype = None
+            lib.traj_oracle_normals.argtypes = [ctypes.c_uint64, ctypes.c_int32, ctypes.c_int64, _dp, _dp]
+            lib.traj_oracle_normals.restype = None
             _LIBS["traj"] = lib
         lib = _LIBS["traj"]
     ini = [_f64(a).ravel() for a in (x0, y0, vx0, vy0)]
     count = ini[0].shape[0]
     out = {k: np.zeros((count, n)) for k in FIELDS}
-    rc = lib.traj_oracle_generate(int(well), float(kappa), float(length), float(gamma), float(dt), count, n, n,
+    rc = lib.traj_oracle_generate(int(well), float(kappa), float(length), float(gamma), float(dt), float(sigma),
+                                  int(seed), count, n, n,
                                   *[_ptr(a) for a in ini], *[_ptr(out[k]) for k in FIELDS])
     if rc != 0:
         raise ValueError("traj_oracle_generate: invalid arguments")

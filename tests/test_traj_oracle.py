@@ -101,3 +101,76 @@ def test_against_the_independent_python_integrator(oracle_mod):
                             [tr["vx"][0]], [tr["vy"][0]])
     for k in ("x", "y", "vx", "vy", "ax", "ay", "dz"):
         np.testing.assert_allclose(o[k][0], tr[k], rtol=2e-10, atol=1e-12 * np.max(np.abs(tr[k])), err_msg=k)
+
+
+# --------------------------------------------------------------------------- well 2: harmonic + scattering kicks
+WP = 2 * math.pi / 7e-6                                               # configs 2 / 4: 7 um period
+
+
+def test_philox_known_answers(oracle_mod):
+    """tests/golden/philox4x32_10_kat.txt: the published known-answer vectors of Philox4x32-10."""
+    from pathlib import Path
+    rows = [ln.split() for ln in (Path(__file__).parent / "golden" / "philox4x32_10_kat.txt").read_text().splitlines()
+            if ln and not ln.startswith("#")]
+    assert len(rows) == 3
+    for r in rows:
+        v = [int(w, 16) for w in r]
+        assert [int(o) for o in oracle_mod.philox4x32_10(v[:4], v[4:6])] == v[6:]
+
+
+def test_kick_normals_are_standard_normal(oracle_mod):
+    a, b = oracle_mod.kick_normals(seed=11, particle=5, n=400000)
+    for v in (a, b):
+        assert abs(v.mean()) < 5e-3 and abs(v.std() - 1) < 5e-3
+        assert abs(np.mean(np.abs(v) > 2) - 0.0455) < 2e-3               # two-sigma tail of a Gaussian
+        assert abs(np.mean(v ** 4) - 3) < 0.05                           # kurtosis
+    assert abs(np.corrcoef(a, b)[0, 1]) < 5e-3 and abs(np.corrcoef(a[1:], a[:-1])[0, 1]) < 5e-3
+    c, _ = oracle_mod.kick_normals(seed=11, particle=6, n=1000)          # another particle: another stream
+    assert not np.allclose(c, a[:1000])
+
+
+def test_scattering_well_without_kicks_is_exact_harmonic_motion(oracle_mod):
+    """sigma = 0: the step is an exact rotation, so x = A sin(w t + phi) to rounding, for any dt."""
+    A, ph = 0.7e-10, 1.1
+    o = oracle_mod.generate(2, WP * WP, 1.0, 9784.7, 7e-9, 5000, [A * math.sin(ph)], [0.0],
+                            [A * WP * math.cos(ph)], [1e-6], sigma=0.0, seed=1)
+    t = o["t"][0]
+    np.testing.assert_allclose(o["x"][0], A * np.sin(WP * t + ph), rtol=0, atol=1e-12 * A)
+    np.testing.assert_allclose(o["vx"][0], A * WP * np.cos(WP * t + ph), rtol=0, atol=1e-12 * A * WP)
+    np.testing.assert_allclose(o["ax"][0], -WP * WP * o["x"][0], rtol=1e-14)
+    np.testing.assert_allclose(o["y"][0], 1e-6 * t, rtol=1e-13)
+    assert np.all(o["ay"] == 0)
+
+
+def test_scattering_well_against_numpy_recurrence(oracle_mod):
+    """The kicked recurrence re-implemented in numpy longdouble from the recipe,
+    fed with the oracle's own normals: pins the bookkeeping (kick / dt in the acceleration of the kicked
+    sample, Q15; trapezoid y and dz; az)."""
+    LD = np.longdouble
+    n, dt, sig, seed = 3000, 7e-9, 2e-7, 21
+    x0, v0, vy0 = 0.3e-10, 0.5e-10 * WP, -1e-7
+    o = oracle_mod.generate(2, WP * WP, 1.0, 9784.7, dt, n, [x0, -x0], [0.0, 1e-11], [v0, v0], [vy0, 0.0],
+                            sigma=sig, seed=seed)
+    for p, (xi, vi, yi, vyi) in enumerate([(x0, v0, 0.0, vy0), (-x0, v0, 1e-11, 0.0)]):
+        a, b = (v.astype(LD) for v in oracle_mod.kick_normals(seed, p, n + 1))
+        a[0] = b[0] = 0
+        wp, h = LD(WP), LD(dt)
+        c, s = np.cos(wp * h), np.sin(wp * h)
+        x, u = np.empty(n, LD), np.empty(n, LD)
+        x[0], u[0] = xi, LD(vi) / wp
+        for k in range(1, n):
+            x[k] = c * x[k - 1] + s * u[k - 1]
+            u[k] = c * u[k - 1] - s * x[k - 1] + LD(sig) / wp * a[k]
+        vx = u * wp
+        vy = LD(vyi) + LD(sig) * np.cumsum(b[:n])
+        y = LD(yi) + np.concatenate([[LD(0)], np.cumsum((vy[1:] + vy[:-1]) / 2 * h)])
+        ax = -wp * wp * x + LD(sig) * a[:n] / h
+        ay = LD(sig) * b[:n] / h
+        dvz = -(vx * vx + vy * vy) / 2
+        dz = np.concatenate([[LD(0)], np.cumsum((dvz[1:] + dvz[:-1]) / 2 * h)])
+        ref = dict(x=x, vx=vx, vy=vy, y=y, ax=ax, ay=ay, dvz=dvz, dz=dz, az=-(vx * ax + vy * ay))
+        for k, v in ref.items():
+            np.testing.assert_allclose(o[k][p], v.astype(np.float64), rtol=1e-11,
+                                       atol=1e-13 * float(np.max(np.abs(v))), err_msg=f"particle {p} {k}")
+    # Q15: the accelerations reproduce the velocity change sample-wise to O(dt): sum(ay dt) = vy - vy0 exactly
+    np.testing.assert_allclose(np.cumsum(o["ay"][0]) * dt, o["vy"][0] - vy0, rtol=1e-9, atol=1e-18)
