@@ -132,22 +132,29 @@ int rad_angular_sum(const double *cube, const rad_grid *grid, double d_solid_ang
 
 /* Trajectories of `count` particles in a static synthetic well, generated on the device in the SoA
  * layout the calls above read -- the paper's outlook "many particle trajectories evaluated in parallel
- * on the GPU", for the wells of BASELINE.json configs 3 and 5 (the paper's own solver
+ * on the GPU", for the wells of BASELINE.json configs 2-5 (the paper's own solver
  * needs potential tables that are not available).  Fixed-step velocity Verlet:
  *   a_k = A(r_k), v_h = v_k + dt/2 a_k, r_{k+1} = r_k + dt v_h, v_{k+1} = v_h + dt/2 A(r_{k+1})
  *   RAD_WELL_COSINE:     A_x = -kappa sin(2 pi x / length), A_y = 0
  *   RAD_WELL_AXIAL_EXP:  A = -kappa (r/|r|) exp(-|r| / length), A(0) = 0
+ * RAD_WELL_HARMONIC_MS (planar harmonic well with multiple-scattering kicks, the recipe of configs 2 and 4;
+ * kappa = w_p^2, length unused but > 0): exact rotation of (x, u = vx / w_p) by w_p dt, then Gaussian kicks
+ *   x_{k+1} = c x_k + s u_k,  u_{k+1} = c u_k - s x_k + (sigma/w_p) xi1_{k+1},  vy_{k+1} = vy_k + sigma xi2_{k+1},
+ *   ax_k = -w_p^2 x_k + sigma xi1_k/dt, ay_k = sigma xi2_k/dt (xi_0 = 0), y = cumulative trapezoid of vy;
+ *   xi1, xi2 of (particle p, step k) = Box-Muller of the uniforms (r + 1/2) 2^-32 from the first two words of
+ *   Philox4x32-10 with counter (k low, k high, p, 0) and key (seed low, seed high): reproducible anywhere.
+ * sigma and seed are ignored by the two deterministic wells.
  * and t_k = k dt, dvz = -(vx^2 + vy^2)/2, dz = cumulative trapezoid of dvz (dz_0 = 0),
  * az = -(vx ax + vy ay) (leading-order relations), gamma_k = gamma.
  * x0, y0, vx0, vy0: DEVICE arrays of `count` initial values.  out: DEVICE arrays [count][stride], the
  * first n entries of each row are written (pass them to rad_ensemble_sum as a rad_traj_batch with
  * the same stride).  One thread per particle: meant for many particles. */
-typedef enum { RAD_WELL_COSINE = 0, RAD_WELL_AXIAL_EXP = 1 } rad_well;
+typedef enum { RAD_WELL_COSINE = 0, RAD_WELL_AXIAL_EXP = 1, RAD_WELL_HARMONIC_MS = 2 } rad_well;
 typedef struct {
     double *t, *dz, *x, *y, *vx, *vy, *dvz, *ax, *ay, *az, *gamma;
 } rad_traj_buffers;
 int rad_generate_trajectories(rad_well well, double kappa, double length, double gamma, double dt,
-                              int32_t count, int64_t n, int64_t stride,
+                              double sigma, uint64_t seed, int32_t count, int64_t n, int64_t stride,
                               const double *x0, const double *y0, const double *vx0, const double *vy0,
                               const rad_traj_buffers *out, void *cuda_stream);
 

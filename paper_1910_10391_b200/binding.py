@@ -98,7 +98,7 @@ def load_library() -> ctypes.CDLL:
     lib.rad_plan_kernel.restype = ctypes.c_int
     lib.rad_plan_describe.argtypes = [i32, i64, i32, i32, i32, ctypes.c_int, ctypes.POINTER(ctypes.c_int32)]
     lib.rad_plan_describe.restype = ctypes.c_int
-    lib.rad_generate_trajectories.argtypes = ([ctypes.c_int] + [dbl] * 4 + [i32, i64, i64] + [vp] * 4
+    lib.rad_generate_trajectories.argtypes = ([ctypes.c_int] + [dbl] * 5 + [ctypes.c_uint64, i32, i64, i64] + [vp] * 4
                                               + [ctypes.POINTER(_TrajBuffers), vp])
     lib.rad_generate_trajectories.restype = ctypes.c_int
     lib.rad_workspace_bytes.argtypes = [i32, i64, i32, i32, i32]
@@ -259,11 +259,12 @@ def rad_angular_sum(cube, omega, thx, thy, d_solid_angle: float, theta_cut: floa
     return out
 
 
-WELL_COSINE, WELL_AXIAL_EXP = 0, 1
+WELL_COSINE, WELL_AXIAL_EXP, WELL_HARMONIC_MS = 0, 1, 2
 
 
 def rad_generate_trajectories(well: int, kappa: float, length: float, gamma: float, dt: float, n: int,
-                              x0, y0, vx0, vy0, out: dict | None = None, stream=None) -> dict:
+                              x0, y0, vx0, vy0, out: dict | None = None, stream=None, sigma: float = 0.0,
+                              seed: int = 0) -> dict:
     """`count` particles in a synthetic well, generated on the device (PAPER.md:233 outlook): FIELDS ->
     (count, n) CUDA tensors ready for rad_ensemble_sum."""
     ini = [_dev(a, name) for a, name in ((x0, "x0"), (y0, "y0"), (vx0, "vx0"), (vy0, "vy0"))]
@@ -277,7 +278,8 @@ def rad_generate_trajectories(well: int, kappa: float, length: float, gamma: flo
     if any(tuple(t.shape) != (count, stride) for t in ts):
         raise ValueError("out tensors must share one (count, stride) shape")
     bufs = _TrajBuffers(*[t.data_ptr() for t in ts])
-    _check(load_library().rad_generate_trajectories(int(well), float(kappa), float(length), float(gamma), float(dt), count,
+    _check(load_library().rad_generate_trajectories(int(well), float(kappa), float(length), float(gamma), float(dt),
+                                                    float(sigma), int(seed), count,
                                          int(n), int(stride), *[a.data_ptr() for a in ini], ctypes.byref(bufs),
                                          _stream_ptr(stream)))
     return out

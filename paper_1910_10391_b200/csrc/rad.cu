@@ -775,12 +775,13 @@ int rad_angular_sum(const double *cube, const rad_grid *grid, double d_solid_ang
 }
 
 int rad_generate_trajectories(rad_well well, double kappa, double length, double gamma, double dt,
-                              int32_t count, int64_t n, int64_t stride,
+                              double sigma, uint64_t seed, int32_t count, int64_t n, int64_t stride,
                               const double *x0, const double *y0, const double *vx0, const double *vy0,
                               const rad_traj_buffers *out, void *cuda_stream) {
     if (!out || !x0 || !y0 || !vx0 || !vy0 || count < 1 || n < 2 || stride < n) return RAD_EINVAL;
-    if (well != RAD_WELL_COSINE && well != RAD_WELL_AXIAL_EXP) return RAD_EINVAL;
-    if (!(dt > 0.0) || !(length > 0.0) || !(gamma >= 1.0)) return RAD_EDOMAIN;
+    if (well != RAD_WELL_COSINE && well != RAD_WELL_AXIAL_EXP && well != RAD_WELL_HARMONIC_MS) return RAD_EINVAL;
+    if (!(dt > 0.0) || !(length > 0.0) || !(gamma >= 1.0) || !(sigma >= 0.0)) return RAD_EDOMAIN;
+    if (well == RAD_WELL_HARMONIC_MS && !(kappa > 0.0)) return RAD_EDOMAIN;
     double *arrs[11] = {out->t, out->dz, out->x, out->y, out->vx, out->vy, out->dvz, out->ax, out->ay, out->az,
                         out->gamma};
     for (double *p : arrs)
@@ -788,7 +789,9 @@ int rad_generate_trajectories(rad_well well, double kappa, double length, double
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const TrajOut o{out->t, out->dz, out->x, out->y, out->vx, out->vy, out->dvz, out->ax, out->ay, out->az, out->gamma};
     const unsigned blocks = (unsigned)((count + 127) / 128);
-    if (well == RAD_WELL_COSINE)
+    if (well == RAD_WELL_HARMONIC_MS)
+        rad_traj_ms_kernel<<<blocks, 128, 0, st>>>(kappa, gamma, dt, sigma, seed, count, n, stride, x0, y0, vx0, vy0, o);
+    else if (well == RAD_WELL_COSINE)
         rad_traj_kernel<0><<<blocks, 128, 0, st>>>(kappa, length, gamma, dt, count, n, stride, x0, y0, vx0, vy0, o);
     else
         rad_traj_kernel<1><<<blocks, 128, 0, st>>>(kappa, length, gamma, dt, count, n, stride, x0, y0, vx0, vy0, o);

@@ -25,6 +25,69 @@ __device__ __forceinline__ void well_accel(double kappa, double L, double x, dou
     }
 }
 
+// Philox4x32-10 (Salmon, Moraes, Dror, Shaw, SC'11): counter-based, so particle p / step k draw the same
+// numbers wherever and in whatever order they are evaluated.
+__device__ __forceinline__ uint2 philox4x32_10_first2(uint32_t c0, uint32_t c1, uint32_t c2, uint32_t c3,
+                                                      uint32_t k0, uint32_t k1) {
+#pragma unroll
+    for (int r = 0; r < 10; ++r) {
+        const uint32_t h0 = __umulhi(0xD2511F53u, c0), l0 = 0xD2511F53u * c0;
+        const uint32_t h1 = __umulhi(0xCD9E8D57u, c2), l1 = 0xCD9E8D57u * c2;
+        const uint32_t n0 = h1 ^ c1 ^ k0, n2 = h0 ^ c3 ^ k1;
+        c0 = n0; c1 = l1; c2 = n2; c3 = l0;
+        k0 += 0x9E3779B9u; k1 += 0xBB67AE85u;
+    }
+    return make_uint2(c0, c1);
+}
+
+// the two standard normals of (particle p, step k): Box-Muller of (r + 1/2) 2^-32
+__device__ __forceinline__ void kick_normals(uint64_t seed, int p, int64_t k, double &xi1, double &xi2) {
+    const uint2 r = philox4x32_10_first2((uint32_t)k, (uint32_t)((uint64_t)k >> 32), (uint32_t)p, 0u,
+                                         (uint32_t)seed, (uint32_t)(seed >> 32));
+    const double u1 = ((double)r.x + 0.5) * 0x1p-32, u2 = ((double)r.y + 0.5) * 0x1p-32;
+    const double rho = sqrt(-2.0 * log(u1));
+    double sn, cs;
+    sincospi(2.0 * u2, &sn, &cs);
+    xi1 = rho * cs;
+    xi2 = rho * sn;
+}
+
+// planar harmonic well (kappa = w_p^2) with Gaussian multiple-scattering kicks of standard deviation sigma on
+// v_x, v_y after every step: exact rotation of (x, v_x / w_p) by w_p dt, then the kick (recipe of configs 2, 4)
+__global__ void __launch_bounds__(128)
+rad_traj_ms_kernel(double kappa, double gamma, double dt, double sigma, uint64_t seed, int count, int64_t n,
+                   int64_t stride, const double *x0, const double *y0, const double *vx0, const double *vy0,
+                   TrajOut o) {
+    const int p = blockIdx.x * blockDim.x + threadIdx.x;
+    if (p >= count) return;
+    const int64_t base = (int64_t)p * stride;
+    const double wp = sqrt(kappa), hh = 0.5 * dt;
+    double sn, cs;
+    sincos(wp * dt, &sn, &cs);
+    double rx = x0[p], ry = y0[p], u = vx0[p] / wp, wy = vy0[p];
+    double dzk = 0.0, dvz_prev = 0.0, vy_prev = wy, xi1 = 0.0, xi2 = 0.0;
+    for (int64_t k = 0; k < n; ++k) {
+        const double vxk = u * wp;
+        const double dvzk = -0.5 * (vxk * vxk + wy * wy);
+        if (k > 0) { dzk += (dvzk + dvz_prev) * hh; ry += (wy + vy_prev) * hh; }
+        dvz_prev = dvzk; vy_prev = wy;
+        const double a_x = -kappa * rx + sigma * xi1 / dt, a_y = sigma * xi2 / dt;
+        const int64_t i = base + k;
+        o.t[i] = dt * (double)k;
+        o.x[i] = rx;    o.y[i] = ry;
+        o.vx[i] = vxk;  o.vy[i] = wy;
+        o.ax[i] = a_x;  o.ay[i] = a_y;
+        o.dvz[i] = dvzk; o.dz[i] = dzk;
+        o.az[i] = -(vxk * a_x + wy * a_y);
+        o.gamma[i] = gamma;
+        kick_normals(seed, p, k + 1, xi1, xi2);
+        const double xn = cs * rx + sn * u;
+        u = cs * u - sn * rx + sigma / wp * xi1;
+        rx = xn;
+        wy += sigma * xi2;
+    }
+}
+
 template <int WELL>
 __global__ void __launch_bounds__(128)
 rad_traj_kernel(double kappa, double L, double gamma, double dt, int count, int64_t n, int64_t stride,

@@ -14,7 +14,8 @@ pytestmark = pytest.mark.gpu
 
 EPS = 2.0 ** -53
 WELLS = {0: dict(kappa=math.pi * 5e-5 ** 2 / (2 * 1.92e-10), L=1.92e-10, gamma=39139.0, th=5e-5),     # config 3
-         1: dict(kappa=3e-5 ** 2 / (2 * 0.3e-10), L=0.3e-10, gamma=97847.0, th=3e-5)}                  # config 5
+         1: dict(kappa=3e-5 ** 2 / (2 * 0.3e-10), L=0.3e-10, gamma=97847.0, th=3e-5),                  # config 5
+         2: dict(kappa=(2 * math.pi / 7e-6) ** 2, L=1.0, gamma=9784.7, th=0.0, sigma=2e-7, dt=7e-9)}   # configs 2, 4
 
 
 @pytest.fixture(scope="module")
@@ -31,6 +32,9 @@ def rad():
 def initial_conditions(well, count, seed):
     rng = np.random.Generator(np.random.PCG64(seed))
     w = WELLS[well]
+    if well == 2:                                      # amplitude uniform in [0, 0.96 A], phase uniform
+        amp, ph = rng.uniform(0, 0.96e-10, count), rng.uniform(0, 2 * np.pi, count)
+        return amp * np.sin(ph), np.zeros(count), amp * math.sqrt(w["kappa"]) * np.cos(ph), np.zeros(count)
     if well == 0:
         return (rng.uniform(-0.5 * w["L"], 0.5 * w["L"], count), np.zeros(count),
                 rng.uniform(-w["th"], w["th"], count), np.zeros(count))
@@ -39,16 +43,17 @@ def initial_conditions(well, count, seed):
     return r * np.cos(a), r * np.sin(a), v * np.cos(b), v * np.sin(b)
 
 
-@pytest.mark.parametrize("well", [0, 1])
+@pytest.mark.parametrize("well", [0, 1, 2])
 def test_generator_matches_oracle(rad, oracle_mod, well):
     import torch
     w = WELLS[well]
-    count, n, stride, dt = 300, 20000, 20003, 1e-9
+    count, n, stride, dt = 300, 20000, 20003, w.get("dt", 1e-9)
+    sigma, seed = w.get("sigma", 0.0), 4242
     ini = initial_conditions(well, count, seed=40 + well)
     dev = [torch.from_numpy(a).cuda() for a in ini]
     out = {k: torch.full((count, stride), -7.0, dtype=torch.float64, device="cuda") for k in rad.FIELDS}
-    rad.rad_generate_trajectories(well, w["kappa"], w["L"], w["gamma"], dt, n, *dev, out=out)
-    ref = oracle_mod.generate(well, w["kappa"], w["L"], w["gamma"], dt, n, *ini)
+    rad.rad_generate_trajectories(well, w["kappa"], w["L"], w["gamma"], dt, n, *dev, out=out, sigma=sigma, seed=seed)
+    ref = oracle_mod.generate(well, w["kappa"], w["L"], w["gamma"], dt, n, *ini, sigma=sigma, seed=seed)
     worst = 0.0
     for k in rad.FIELDS:
         got = out[k].cpu().numpy()
@@ -69,14 +74,16 @@ def test_generator_edge_cases(rad):
     assert all(torch.all(out[k] == 0) for k in ("x", "y", "vx", "vy", "ax", "ay", "az", "dz", "dvz"))
     assert out["t"].cpu().tolist() == [[0.0, 1e-9]] and torch.all(out["gamma"] == w["gamma"])
     with pytest.raises(rad.RadError):
-        rad.rad_generate_trajectories(2, 1.0, 1.0, 10.0, 1e-9, 10, z, z, z, z)
+        rad.rad_generate_trajectories(3, 1.0, 1.0, 10.0, 1e-9, 10, z, z, z, z)
+    with pytest.raises(rad.RadError):
+        rad.rad_generate_trajectories(2, 1.0, 1.0, 10.0, 1e-9, 10, z, z, z, z, sigma=-1.0)
     with pytest.raises(rad.RadError):
         rad.rad_generate_trajectories(0, 1.0, 1.0, 10.0, 1e-9, 1, z, z, z, z)
     with pytest.raises(rad.RadError):
         rad.rad_generate_trajectories(0, 1.0, 1.0, 10.0, -1e-9, 10, z, z, z, z)
 
 
-@pytest.mark.parametrize("well,model", [(0, 2), (1, 1)])
+@pytest.mark.parametrize("well,model", [(0, 2), (1, 1), (2, 0)])
 def test_generated_ensemble_feeds_the_spectrum_on_the_device(rad, oracle_mod, well, model):
     """Trajectories generated on the device go straight into rad_ensemble_sum (no host round trip); the
     spectrum is compared with the oracle evaluated on a host copy of the same trajectories."""
@@ -86,12 +93,15 @@ def test_generated_ensemble_feeds_the_spectrum_on_the_device(rad, oracle_mod, we
     w = WELLS[well]
     count, n = 24, 6000
     ini = initial_conditions(well, count, seed=50 + well)
-    batch = rad.rad_generate_trajectories(well, w["kappa"], w["L"], w["gamma"], 1e-9, n,
-                                          *[torch.from_numpy(a).cuda() for a in ini])
+    batch = rad.rad_generate_trajectories(well, w["kappa"], w["L"], w["gamma"], w.get("dt", 1e-9), n,
+                                          *[torch.from_numpy(a).cuda() for a in ini],
+                                          sigma=w.get("sigma", 0.0), seed=99)
     E = w["gamma"] * workloads.ME_EV
     lam = workloads.HBARC_EV_M / E
     omega = 0.6 * E * (np.arange(16) + 1.0) / 16 / workloads.HBARC_EV_M
     half = w["th"] + 3.0 / w["gamma"]
+    if well == 2:                                      # config-2 style grid: classical, around 2 gamma^2 w_p
+        omega = 2 * w["gamma"] ** 2 * math.sqrt(w["kappa"]) * np.geomspace(0.05, 10, 16)
     th = -half + 2 * half * np.arange(16) / 15
     g = [torch.from_numpy(a).cuda() for a in (omega, th, th)]
     nvec = np.full(count, n, dtype=np.int64)
