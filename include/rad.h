@@ -111,6 +111,19 @@ int rad_ensemble_sum(const rad_traj_batch *batch, const rad_grid *grid, rad_mode
                      const double *hbarc_over_E, int accumulate, double *out,
                      void *workspace, size_t workspace_bytes, void *cuda_stream);
 
+/* dI/dw of an ensemble WITHOUT materialising the whole cube (3000^2 angles x 100 omegas
+ * "approach the limit" of GPU memory at one double per integral): the grid is processed in slabs of omegas
+ * whose cube (<= ~256 MB) lives in the workspace, each slab summed over the angles as rad_angular_sum does.
+ * spectrum: n_omega doubles (device), overwritten.  workspace: DEVICE, 256-byte aligned, REQUIRED here, at
+ * least rad_angular_spectrum_workspace_bytes() bytes.  batch->n and hbarc_over_E are HOST arrays as in
+ * rad_ensemble_sum (count = 1 for a single trajectory).  Same values as cube + rad_angular_sum up to the
+ * rounding of a different time / trajectory split (a slab has its own launch plan). */
+int rad_angular_spectrum(const rad_traj_batch *batch, const rad_grid *grid, rad_model model,
+                         const double *hbarc_over_E, double d_solid_angle, double theta_cut, double *spectrum,
+                         void *workspace, size_t workspace_bytes, void *cuda_stream);
+size_t rad_angular_spectrum_workspace_bytes(int32_t count, int64_t n_max, int32_t n_omega, int32_t n_thx,
+                                            int32_t n_thy);
+
 /* One long trajectory cut into sections with their own energy -- the paper's treatment of energy
  * loss: "the total spectrum is then the sum of the spectra from each section".
  * out[m] (+)= sum over s (ascending) of the spectrum of samples start[s] .. start[s+1], BOTH included:

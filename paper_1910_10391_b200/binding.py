@@ -20,7 +20,8 @@ EXPORTS = ("rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_sectio
            "rad_workspace_bytes", "rad_eval_host", "rad_ensemble_sum_host",
            "rad_measure_fp64_peak", "rad_launch_count", "rad_strerror",
            "rad_profile_enable", "rad_profile_last", "rad_set_kernel", "rad_plan_kernel",
-           "rad_generate_trajectories", "rad_plan_describe")
+           "rad_generate_trajectories", "rad_plan_describe", "rad_angular_spectrum",
+           "rad_angular_spectrum_workspace_bytes")
 
 _dp = ctypes.POINTER(ctypes.c_double)
 _lib = None
@@ -96,6 +97,11 @@ def load_library() -> ctypes.CDLL:
     lib.rad_set_kernel.restype = ctypes.c_int
     lib.rad_plan_kernel.argtypes = [i32, i32, i32, ctypes.c_int]
     lib.rad_plan_kernel.restype = ctypes.c_int
+    lib.rad_angular_spectrum.argtypes = [ctypes.POINTER(_Batch), ctypes.POINTER(_Grid), ctypes.c_int, vp, dbl, dbl,
+                                         vp, vp, sz, vp]
+    lib.rad_angular_spectrum.restype = ctypes.c_int
+    lib.rad_angular_spectrum_workspace_bytes.argtypes = [i32, i64, i32, i32, i32]
+    lib.rad_angular_spectrum_workspace_bytes.restype = sz
     lib.rad_plan_describe.argtypes = [i32, i64, i32, i32, i32, ctypes.c_int, ctypes.POINTER(ctypes.c_int32)]
     lib.rad_plan_describe.restype = ctypes.c_int
     lib.rad_generate_trajectories.argtypes = ([ctypes.c_int] + [dbl] * 5 + [ctypes.c_uint64, i32, i64, i64] + [vp] * 4
@@ -297,6 +303,32 @@ def rad_sum_cubes(cubes, accumulate: bool = False, out=None, stream=None):
         raise ValueError("out has the wrong number of elements")
     _check(load_library().rad_sum_cubes(cubes.data_ptr(), count, m, 1 if accumulate else 0, out.data_ptr(),
                                         _stream_ptr(stream)))
+    return out
+
+
+def rad_angular_spectrum(batch: dict, n, omega, thx, thy, d_solid_angle: float, theta_cut: float = 0.0,
+                         model: int = CLASSICAL, hbarc_over_E=None, out=None, workspace=None, stream=None):
+    """dI/dw of an ensemble, slab by slab, without the whole cube in memory."""
+    ts = [_dev(batch[k], k) for k in FIELDS]
+    count, stride = ts[0].shape
+    n_host = np.ascontiguousarray(n, dtype=np.int64)
+    if n_host.shape != (count,):
+        raise ValueError("n must have shape (count,)")
+    lam = None
+    if hbarc_over_E is not None:
+        lam = np.ascontiguousarray(np.broadcast_to(np.asarray(hbarc_over_E, dtype=np.float64), (count,)))
+    b = _Batch(count, stride, n_host.ctypes.data, *[t.data_ptr() for t in ts])
+    g = _grid_struct(_dev(omega, "omega"), _dev(thx, "thx"), _dev(thy, "thy"))
+    lib = load_library()
+    if workspace is None:
+        need = lib.rad_angular_spectrum_workspace_bytes(count, int(n_host.max()), omega.numel(), thx.numel(), thy.numel())
+        workspace = torch.empty(need, dtype=torch.uint8, device=omega.device)
+    ws, nb = _ws_args(workspace)
+    if out is None:
+        out = torch.empty(omega.numel(), dtype=torch.float64, device=omega.device)
+    _check(lib.rad_angular_spectrum(ctypes.byref(b), ctypes.byref(g), int(model),
+                                    lam.ctypes.data if lam is not None else None, float(d_solid_angle),
+                                    float(theta_cut), _dev(out, "out").data_ptr(), ws, nb, _stream_ptr(stream)))
     return out
 
 

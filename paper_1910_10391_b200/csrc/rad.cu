@@ -774,6 +774,47 @@ int rad_angular_sum(const double *cube, const rad_grid *grid, double d_solid_ang
     return RAD_OK;
 }
 
+// omegas per slab of rad_angular_spectrum: the slab cube stays below ~256 MB, whole 16-omega tiles
+static int spectrum_slab(int n_omega, int n_thx, int n_thy) {
+    const int64_t per_omega = (int64_t)n_thx * n_thy * 8;
+    int64_t k = std::max<int64_t>(16, ((int64_t)256 << 20) / per_omega / 16 * 16);
+    return (int)std::min<int64_t>(k, n_omega);
+}
+
+size_t rad_angular_spectrum_workspace_bytes(int32_t count, int64_t n_max, int32_t n_omega, int32_t n_thx,
+                                            int32_t n_thy) {
+    if (count < 1 || n_max < 2 || n_omega < 1 || n_thx < 1 || n_thy < 1) return 0;
+    const int k = spectrum_slab(n_omega, n_thx, n_thy);
+    const size_t inner = rad_workspace_bytes(count, n_max, k, n_thx, n_thy);
+    return align_up(inner, 256) + align_up((size_t)k * n_thx * n_thy * 8, 256);
+}
+
+int rad_angular_spectrum(const rad_traj_batch *batch, const rad_grid *grid, rad_model model,
+                         const double *hbarc_over_E, double d_solid_angle, double theta_cut, double *spectrum,
+                         void *workspace, size_t workspace_bytes, void *cuda_stream) {
+    if (!batch || !grid_ok(grid) || !spectrum || !workspace) return RAD_EINVAL;
+    if (reinterpret_cast<uintptr_t>(workspace) & 255) return RAD_EINVAL;
+    int64_t n_max = 0;
+    if (!batch->n || batch->count < 1) return RAD_EINVAL;
+    for (int p = 0; p < batch->count; ++p) n_max = std::max(n_max, batch->n[p]);
+    if (n_max < 2) return RAD_EINVAL;
+    const int k = spectrum_slab(grid->n_omega, grid->n_thx, grid->n_thy);
+    const size_t inner = align_up(rad_workspace_bytes(batch->count, n_max, k, grid->n_thx, grid->n_thy), 256);
+    const size_t cube_bytes = align_up((size_t)k * grid->n_thx * grid->n_thy * 8, 256);
+    if (workspace_bytes < inner + cube_bytes) return RAD_ENOSPACE;
+    double *cube = reinterpret_cast<double *>(static_cast<char *>(workspace) + inner);
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    for (int w0 = 0; w0 < grid->n_omega; w0 += k) {    // one slab of omegas at a time: cube of the slab, then its sum
+        const int kw = std::min(k, grid->n_omega - w0);
+        rad_grid slab{kw, grid->n_thx, grid->n_thy, grid->omega + w0, grid->thx, grid->thy};
+        int rc = run_batch(batch, batch->n, nullptr, &slab, (int)model, hbarc_over_E, 0, cube, workspace, inner, st);
+        if (rc != RAD_OK) return rc;
+        rc = rad_angular_sum(cube, &slab, d_solid_angle, theta_cut, spectrum + w0, cuda_stream);
+        if (rc != RAD_OK) return rc;
+    }
+    return RAD_OK;
+}
+
 int rad_generate_trajectories(rad_well well, double kappa, double length, double gamma, double dt,
                               double sigma, uint64_t seed, int32_t count, int64_t n, int64_t stride,
                               const double *x0, const double *y0, const double *vx0, const double *vy0,

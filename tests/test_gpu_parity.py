@@ -561,3 +561,31 @@ def test_cfg4_full_size_sampled(rad, oracle_mod):
     w, nx, ny = workloads.points_of(we, idx)
     ref = oracle_mod.ensemble_points(we.batch, we.n, w, nx, ny)
     assert_parity(cube, ref, idx, label="cfg4 FULL")
+
+
+def test_angular_spectrum_in_slabs(rad, oracle_mod):
+    """rad_angular_spectrum: dI/dw slab by slab (3 slabs of <= 16 omegas here) without the 460 MB cube of the
+    whole grid; equals cube + rad_angular_sum, and the oracle's sum on a small grid."""
+    import torch
+    wl = workloads.make("cfg2", n=120, n_omega=40, n_th=1200, seed=19)
+    g = dev_grid(wl)
+    d_om = (wl.thx[1] - wl.thx[0]) * (wl.thy[1] - wl.thy[0])
+    cut = 2.5 / wl.meta["gamma"]
+    b = {k: v[None, :].contiguous() for k, v in dev_dict(wl.traj).items()}
+    n = np.array([120], dtype=np.int64)
+    assert rad.load_library().rad_angular_spectrum_workspace_bytes(1, 120, 40, 1200, 1200) < 1200 * 1200 * 8 * 20
+    got = rad.rad_angular_spectrum(b, n, *g, d_om, cut).cpu().numpy()
+    cube = rad.rad_classical(dev_dict(wl.traj), *g)
+    want = rad.rad_angular_sum(cube, *g, d_om, cut).cpu().numpy()
+    np.testing.assert_allclose(got, want, rtol=1e-12)
+    del cube
+    torch.cuda.empty_cache()
+    ws = workloads.make("cfg3", n=800, n_omega=9, n_th=7, seed=23)          # small: against the oracle, spin-1/2
+    gs = dev_grid(ws)
+    bs = {k: v[None, :].contiguous() for k, v in dev_dict(ws.traj).items()}
+    got = rad.rad_angular_spectrum(bs, np.array([800]), *gs, 1.0, 0.0, model=SH, hbarc_over_E=ws.hbarc_over_E)
+    ref = oracle_mod.grid(ws.traj, ws.omega, ws.thx, ws.thy, SH, ws.hbarc_over_E).sum((1, 2))
+    np.testing.assert_allclose(got.cpu().numpy(), ref, rtol=1e-9)
+    with pytest.raises(rad.RadError) as e:
+        rad.rad_angular_spectrum(bs, np.array([800]), *gs, 1.0, workspace=torch.empty(1024, dtype=torch.uint8, device="cuda"))
+    assert e.value.code == -4
