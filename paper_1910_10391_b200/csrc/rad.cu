@@ -474,6 +474,13 @@ static int sm_count() {
 
 static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
 
+// Scratch taken from the stream-ordered pool goes back in stream order on every exit path.
+struct PoolScratch {
+    void *p = nullptr;
+    cudaStream_t st = nullptr;
+    ~PoolScratch() { if (p) cudaFreeAsync(p, st); }
+};
+
 // The launch plan is a pure function of the shapes (and the SM count, 148 assumed when no
 // device is visible so that rad_workspace_bytes works on a CPU-only box).
 struct Plan {
@@ -629,7 +636,7 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const int64
                               choose_kernel(g->n_omega, g->n_thx, g->n_thy, nc));
     if (workspace && (reinterpret_cast<uintptr_t>(workspace) & 255)) return RAD_EINVAL;
     if (workspace && workspace_bytes < pl.total) return RAD_ENOSPACE;
-    bool own = false;
+    PoolScratch pool;
     char *ws = static_cast<char *>(workspace);
     if (!ws) {
         // keep freed scratch cached in the device's stream-ordered pool: with the default release
@@ -648,7 +655,7 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const int64
         void *pnew = nullptr;
         CK(cudaMallocAsync(&pnew, pl.total, st));
         ws = static_cast<char *>(pnew);
-        own = true;
+        pool.p = pnew; pool.st = st;
     }
     double *packed = reinterpret_cast<double *>(ws + pl.off_packed);
     int64_t *n_dev = nullptr;
@@ -704,7 +711,6 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const int64
         CK(cudaGetLastError());
         prof_mark(3, st);
     }
-    if (own) CK(cudaFreeAsync(ws, st));
     return RAD_OK;
 }
 
@@ -873,6 +879,8 @@ int rad_ensemble_sum_host(const rad_traj_batch *b, const rad_grid *g, rad_model 
         if (!p) return RAD_EINVAL;
     double *dev = nullptr;
     CK(cudaMallocAsync(reinterpret_cast<void **>(&dev), (11 * tot + ng + M) * sizeof(double), st));
+    PoolScratch pool;
+    pool.p = dev; pool.st = st;
     const double *d[11];
     for (int i = 0; i < 11; ++i) {
         d[i] = dev + i * tot;
@@ -891,6 +899,7 @@ int rad_ensemble_sum_host(const rad_traj_batch *b, const rad_grid *g, rad_model 
         if (e != cudaSuccess) rc = cuda_fail(e, "D2H");
     }
     cudaFreeAsync(dev, st);
+    pool.p = nullptr;
     cudaError_t e = cudaStreamSynchronize(st);
     if (rc == RAD_OK && e != cudaSuccess) rc = cuda_fail(e, "cudaStreamSynchronize");
     return rc;
