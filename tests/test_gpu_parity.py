@@ -235,7 +235,14 @@ def test_host_entry_points(rad, oracle_mod):
     we = workloads.make("cfg4", count=4, n=500, n_omega=6, n_th=3)
     cube = rad.rad_ensemble_sum_host(we.batch, we.n, we.omega, we.thx, we.thy)
     w, nx, ny = oracle_mod.grid_points(we.omega, we.thx, we.thy)
-    assert_parity(cube, oracle_mod.ensemble_points(we.batch, we.n, w, nx, ny), label="host ensemble")
+    ref = oracle_mod.ensemble_points(we.batch, we.n, w, nx, ny)
+    assert_parity(cube, ref, label="host ensemble")
+    # accumulate on the host path: first two trajectories, then the other two added to the same cube
+    part = rad.rad_ensemble_sum_host({k: np.ascontiguousarray(v[:2]) for k, v in we.batch.items()}, we.n[:2],
+                                     we.omega, we.thx, we.thy)
+    both = rad.rad_ensemble_sum_host({k: np.ascontiguousarray(v[2:]) for k, v in we.batch.items()}, we.n[2:],
+                                     we.omega, we.thx, we.thy, accumulate=True, out=part)
+    assert_parity(both, ref, label="host ensemble accumulate")
 
 
 # ------------------------------------------------------------------ angular sum (NEXT-1)
