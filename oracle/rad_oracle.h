@@ -19,7 +19,8 @@
  * Parity pins (tests/test_oracle_pins.py): P1 straight line, P2 transversality,
  * P3 per-angle Parseval, P4 harmonic positions, P5 weak-undulator closed form,
  * P6 brute force of the unexpanded eqs. (1)-(2), P7 variant identities,
- * P8 J by parts, P10 independent numpy re-implementation.
+ * P8 J by parts, P9 quantum synchrotron (Baier-Katkov) limit, P10 independent numpy re-implementation,
+ * symmetries (shifts, mirror, axis swap).
  * PARITY UNPINNED: the choice of quadrature rule (composite trapezoid on the
  * given t_k, reading Q1) is a convention the paper does not state.
  */

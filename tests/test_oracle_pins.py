@@ -398,3 +398,39 @@ def test_mirror_and_axis_swap_symmetry(oracle_mod, model):
     for a, b in (("x", "y"), ("vx", "vy"), ("ax", "ay")):
         tr[a], tr[b] = wl.traj[b].copy(), wl.traj[a].copy()
     np.testing.assert_allclose(oracle_mod.points(tr, om, ny, nx, model, lam), base, rtol=1e-12)
+
+
+# --------------------------------------------------------------------------- P9
+@pytest.mark.parametrize("xi,u", [(0.3, 0.0), (1.0, 0.0), (0.5, 0.3), (1.5, 0.6)])
+def test_p9_quantum_synchrotron_limit(oracle_mod, xi, u):
+    """Circular arc (constant v'_x = a0, deflection +-10/gamma), central in-plane direction n_x = 0, spectrum
+    integrated over n_y: the energy per frequency and per in-plane angle is (dP/dw)/a0 with the textbook
+    (Baier-Katkov) synchrotron spectrum
+        dP/dw = w / (sqrt(3) pi gamma^2) [ int_xi^inf K_5/3 + u^2/(1-u) K_2/3(xi) ]      (units of e^2, c = 1),
+    xi = w*/w_c, w_c = 3 gamma^3 a0 / 2; spin-0: the first term only; u = 0: classical (Jackson 14.91).
+    Pins eq. (10) with its J term and coefficient u^2/2gamma^2 (reading Q4), the substitution w -> w*
+    (eqs. 8-9, reading Q3) and the absolute normalisation against a result the oracle does not contain."""
+    from scipy.integrate import quad
+    from scipy.special import kv
+    gamma, a0, n = 1000.0, 1.0, 40001
+    t = np.linspace(-10.0 / gamma / a0, 10.0 / gamma / a0, n)
+    vx = a0 * t
+    z = np.zeros(n)
+    tr = dict(t=t, x=a0 * t * t / 2, y=z.copy(), vx=vx, vy=z.copy(), ax=np.full(n, a0), ay=z.copy(),
+              dvz=-vx * vx / 2, dz=-a0 * a0 * t ** 3 / 6, az=-a0 * a0 * t, gamma=np.full(n, gamma))
+    w_star = xi * 1.5 * gamma ** 3 * a0
+    om = w_star * (1 - u)
+    lam = u / om
+    ny = np.linspace(-8 / gamma, 8 / gamma, 321)
+    i53 = quad(lambda x: kv(5 / 3, x), xi, np.inf)[0]
+    pref = om / (math.sqrt(3) * math.pi * gamma ** 2) / a0
+    want = {0: None, 1: pref * i53, 2: pref * (i53 + u * u / (1 - u) * kv(2 / 3, xi))}
+    for model in (1, 2):
+        out = oracle_mod.points(tr, np.full(ny.size, om), np.zeros(ny.size), ny, model, lam)
+        got = np.trapezoid(out, ny)
+        assert got == pytest.approx(want[model], rel=1e-3), f"model {model}"
+    if u == 0.0:
+        out = oracle_mod.points(tr, np.full(ny.size, om), np.zeros(ny.size), ny, 0, 0.0)
+        assert np.trapezoid(out, ny) == pytest.approx(want[1], rel=1e-3)
+    else:                                             # the spin term is not small here: it must be there
+        assert want[2] / want[1] - 1 > 0.05
