@@ -136,6 +136,13 @@ int rad_sections_sum(const rad_traj *traj, int32_t n_sections, const int64_t *st
                      rad_model model, const double *hbarc_over_E, int accumulate, double *out,
                      void *workspace, size_t workspace_bytes, void *cuda_stream);
 
+/* Formation length l_f = 2 gamma^2 (E - w)/(E w), in the length unit of omega (c = hbar = 1:
+ * omega in rad/length, u = omega * hbarc_over_E = hbar w / E).  A section handed to rad_sections_sum must be
+ * longer than this.  Host arithmetic only; returns -1 on arguments outside the domain (u >= 1, omega <= 0).
+ * Note: for the paper's own example (50 GeV positron, 5 GeV photon) the formula gives 680 nm, while the
+ * paper prints 71 nm -- the text is at odds with itself there; the formula is what this returns. */
+double rad_formation_length(double gamma, double omega, double hbarc_over_E);
+
 /* dI/dw[i_w] = sum_{i_x,i_y} cube * d_omega_solid, optionally only where
  * n_x^2 + n_y^2 <= theta_cut^2 (theta_cut <= 0: no mask) -- the paper's "final sum over
  * the spatial integrals", done on the device.  `cube` is the output of

@@ -21,7 +21,7 @@ EXPORTS = ("rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_sectio
            "rad_measure_fp64_peak", "rad_launch_count", "rad_strerror",
            "rad_profile_enable", "rad_profile_last", "rad_set_kernel", "rad_plan_kernel",
            "rad_generate_trajectories", "rad_plan_describe", "rad_angular_spectrum",
-           "rad_angular_spectrum_workspace_bytes")
+           "rad_angular_spectrum_workspace_bytes", "rad_formation_length")
 
 _dp = ctypes.POINTER(ctypes.c_double)
 _lib = None
@@ -102,6 +102,8 @@ def load_library() -> ctypes.CDLL:
     lib.rad_angular_spectrum.restype = ctypes.c_int
     lib.rad_angular_spectrum_workspace_bytes.argtypes = [i32, i64, i32, i32, i32]
     lib.rad_angular_spectrum_workspace_bytes.restype = sz
+    lib.rad_formation_length.argtypes = [dbl, dbl, dbl]
+    lib.rad_formation_length.restype = dbl
     lib.rad_plan_describe.argtypes = [i32, i64, i32, i32, i32, ctypes.c_int, ctypes.POINTER(ctypes.c_int32)]
     lib.rad_plan_describe.restype = ctypes.c_int
     lib.rad_generate_trajectories.argtypes = ([ctypes.c_int] + [dbl] * 5 + [ctypes.c_uint64, i32, i64, i64] + [vp] * 4
@@ -412,6 +414,14 @@ def rad_plan_describe(count: int, n_max: int, n_omega: int, n_thx: int, n_thy: i
     plan = (ctypes.c_int32 * 6)()
     _check(load_library().rad_plan_describe(count, n_max, n_omega, n_thx, n_thy, int(model), plan))
     return dict(zip(("kernel", "mode", "tiles", "slices", "t_slices", "chunks"), (int(v) for v in plan)))
+
+
+def rad_formation_length(gamma: float, omega: float, hbarc_over_E: float) -> float:
+    """l_f = 2 gamma^2 (E - w)/(E w), in the length unit of omega; ValueError outside the domain."""
+    v = float(load_library().rad_formation_length(float(gamma), float(omega), float(hbarc_over_E)))
+    if v < 0:
+        raise ValueError("rad_formation_length: need gamma >= 1, omega > 0 and hbar omega < E")
+    return v
 
 
 def rad_profile_enable(on: bool = True) -> None:

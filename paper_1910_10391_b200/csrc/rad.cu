@@ -954,6 +954,12 @@ int rad_plan_kernel(int32_t n_omega, int32_t n_thx, int32_t n_thy, rad_model mod
     return choose_kernel(n_omega, n_thx, n_thy, model == RAD_SPIN_HALF ? 6 : 4) + 1;
 }
 
+double rad_formation_length(double gamma, double omega, double hbarc_over_E) {
+    const double u = omega * hbarc_over_E;            // hbar omega / E
+    if (!(gamma >= 1.0) || !(omega > 0.0) || !(u >= 0.0) || !(u < 1.0)) return -1.0;
+    return 2.0 * gamma * gamma * (1.0 - u) / omega;   // l_f = 2 gamma^2 (E - w) / (E w)
+}
+
 int rad_plan_describe(int32_t count, int64_t n_max, int32_t n_omega, int32_t n_thx, int32_t n_thy, rad_model model,
                       int32_t *plan) {
     if (!plan || count < 1 || n_max < 2 || n_omega < 1 || n_thx < 1 || n_thy < 1) return RAD_EINVAL;

@@ -155,3 +155,20 @@ def test_launch_plans_of_the_baseline_configs(radlib):
     for k in range(1, 60):                           # slices never exceed the work there is
         p = d(k, 300, 16, 16, 16, 0)
         assert p["slices"] <= k * p["chunks"] and p["slices"] >= 1
+
+
+def test_formation_length_of_the_papers_example(radlib):
+    """l_f = 2 gamma^2 (E - w)/(E w); "in the case of a 50 GeV positron emitting a 5 GeV photon
+    l_f = 71 nm".  The formula gives 680 nm for those numbers (tests/golden/formation_length.txt): the paper's
+    printed value is off by a factor 9.6 from its own formula, which DESIGN.md lists as a reading; the library
+    implements the formula."""
+    rows = [ln.split() for ln in (ROOT / "tests" / "golden" / "formation_length.txt").read_text().splitlines()
+            if ln and not ln.startswith("#")]
+    E_eV, w_eV, formula_m, printed_m = (float(v) for v in rows[0])
+    me, hbarc = 0.51099895e6, 1.973269804e-7
+    got = radlib.rad_formation_length(E_eV / me, w_eV / hbarc, hbarc / E_eV)
+    assert got == pytest.approx(formula_m, rel=1e-6)
+    assert got == pytest.approx(2 * (E_eV / me) ** 2 * (E_eV - w_eV) / (E_eV * w_eV) * hbarc, rel=1e-12)
+    assert 9 < got / printed_m < 10                                   # the discrepancy, on record
+    with pytest.raises(ValueError):
+        radlib.rad_formation_length(1e5, 1e18, 1e-17)                 # hbar w >= E
