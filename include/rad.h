@@ -210,8 +210,8 @@ int64_t rad_launch_count(void);
 
 /* Which main kernel later calls use.  0 (default): chosen from the grid shape -- the separable-phasor
  * kernel (e^{i w psi} = T(w, n_x) Y(w, n_y) on a tensor grid, exact because theta^2 = n_x^2 + n_y^2,
- * eq. (7)) when padding the grid to its 16 x 16 x 16 (spin-1/2: 16 x 16 x 8) point tiles
- * wastes less than half of the work, else the direct kernel (one phasor per eval).  1: always direct,
+ * eq. (7)) when the grid fills at least 60 % (spin-1/2: 75 %) of its 16 x 16 x 16 (spin-1/2:
+ * 16 x 16 x 8) point tiles after padding, else the direct kernel (one phasor per eval).  1: always direct,
  * 2: always separable.  Both meet the same tolerance; process-wide; RAD_EINVAL on other values. */
 int rad_set_kernel(int choice);
 
