@@ -37,7 +37,8 @@
  *     the enqueued work and allocates nothing persistent of its own.
  *   - `cuda_stream` is a cudaStream_t (NULL = legacy default stream).  All work is
  *     enqueued on it; no call synchronises the host (the *_host calls do, once, at
- *     the end).
+ *     the end).  With a caller workspace the single-trajectory calls enqueue kernels only
+ *     (no allocation, no host copy), so they can be captured in a CUDA graph and replayed.
  *   - Cube order: out[(i_w * n_thy + i_y) * n_thx + i_x]  (theta_x fastest).
  *   - Return value: RAD_OK (0) or a negative rad_status; nothing throws or aborts.
  *     Not checked (garbage in, NaN/inf out): non-monotone t, q <= 0, non-finite

@@ -596,3 +596,30 @@ def test_angular_spectrum_in_slabs(rad, oracle_mod):
     with pytest.raises(rad.RadError) as e:
         rad.rad_angular_spectrum(bs, np.array([800]), *gs, 1.0, workspace=torch.empty(1024, dtype=torch.uint8, device="cuda"))
     assert e.value.code == -4
+
+
+def test_single_trajectory_call_is_graph_capturable(rad):
+    """With a caller workspace a single-trajectory call only enqueues kernels (no host sync, no allocation, no
+    host copy), so it can be captured in a CUDA graph and replayed; replays reproduce the eager bits."""
+    import torch
+    for shape, kernel in ((dict(n=900, n_omega=16, n_th=6), 1), (dict(n=900, n_omega=32, n_th=16), 2)):
+        wl = workloads.make("cfg2", seed=4, **shape)
+        tr, g = dev_dict(wl.traj), dev_grid(wl)
+        assert rad.rad_plan_kernel(len(wl.omega), len(wl.thx), len(wl.thy), SH) == kernel
+        lam = 0.4 / wl.omega.max()
+        ws = torch.empty(rad.rad_workspace_bytes(1, 900, len(wl.omega), len(wl.thx), len(wl.thy)),
+                         dtype=torch.uint8, device="cuda")
+        out = torch.zeros((len(wl.omega), len(wl.thy), len(wl.thx)), dtype=torch.float64, device="cuda")
+        eager = rad.rad_semiclassical(tr, *g, 1, lam, workspace=ws).clone()        # also warms up the kernels
+        graph = torch.cuda.CUDAGraph()
+        side = torch.cuda.Stream()
+        side.wait_stream(torch.cuda.current_stream())
+        with torch.cuda.stream(side):
+            with torch.cuda.graph(graph, stream=side):
+                rad.rad_semiclassical(tr, *g, 1, lam, out=out, workspace=ws)
+        torch.cuda.current_stream().wait_stream(side)
+        for _ in range(3):
+            out.zero_()
+            graph.replay()
+            torch.cuda.synchronize()
+            assert torch.equal(out, eager)
