@@ -20,9 +20,10 @@
  * P3 per-angle Parseval, P4 harmonic positions, P5 weak-undulator closed form,
  * P6 brute force of the unexpanded eqs. (1)-(2), P7 variant identities,
  * P8 J by parts, P9 quantum synchrotron (Baier-Katkov) limit, P10 independent numpy re-implementation,
- * symmetries (shifts, mirror, axis swap).
- * PARITY UNPINNED: the choice of quadrature rule (composite trapezoid on the
- * given t_k, reading Q1) is a convention the paper does not state.
+ * symmetries (shifts, mirror, axis swap), Q1 (the trapezoid weights, end weights
+ * included: exact closed forms for linear and quadratic integrands on ragged
+ * abscissae), Q6 (gamma_k sample-wise in the integrand, gamma[0] in eq. 10's J
+ * coefficient).  Every function of this file has at least one such pin.
  */
 #ifndef RAD_ORACLE_H
 #define RAD_ORACLE_H

@@ -434,3 +434,95 @@ def test_p9_quantum_synchrotron_limit(oracle_mod, xi, u):
         assert np.trapezoid(out, ny) == pytest.approx(want[1], rel=1e-3)
     else:                                             # the spin term is not small here: it must be there
         assert want[2] / want[1] - 1 > 0.05
+
+
+# --------------------------------------------------------------------------- quadrature rule (Q1) and gamma reading (Q6)
+def _zero_phase_trajectory(t, ax, gamma):
+    """A trajectory whose eq. (3) integrand at omega = 0, n = (0, 0) is the closed form -2 gamma^2 ax:
+    with n = 0, vx = vy = dvz = az = 0 eqs. (3), (6) give D = q = 1/(2 gamma^2), g = 4 gamma^4 and
+    f_x = -D ax g = -2 gamma^2 ax; the phase of eq. (7) is 0 at omega = 0."""
+    tr = {k: np.zeros(len(t)) for k in workloads.FIELDS}
+    tr["t"] = np.asarray(t, dtype=np.float64)
+    tr["ax"] = np.asarray(ax, dtype=np.float64)
+    tr["gamma"] = np.broadcast_to(np.asarray(gamma, dtype=np.float64), tr["t"].shape).copy()
+    return tr
+
+
+def _ragged_times(n, seed):
+    """Non-uniform abscissae with dyadic spacings (exact in double), different first and last steps."""
+    rng = np.random.default_rng(seed)
+    steps = rng.integers(1, 9, size=n - 1).astype(np.float64) * 2.0 ** -10
+    steps[0], steps[-1] = 5 * 2.0 ** -10, 3 * 2.0 ** -10
+    return np.concatenate([[0.25], 0.25 + np.cumsum(steps)])
+
+
+def test_q1_trapezoid_weights_are_exact_for_a_linear_integrand(oracle_mod):
+    """Reading Q1 (the paper only says "points in time"): composite trapezoid on the
+    given t_k.  That rule integrates a LINEAR integrand exactly on any grid, end intervals included:
+    with ax = c0 + c1 t, non-zero at both ends, A_x = -2 gamma^2 [c0 (t_N - t_0) + c1 (t_N^2 - t_0^2)/2].
+    Inputs are dyadic rationals, so the closed form is exact in double and the oracle's long-double sum
+    has no rounding to speak of: tolerance 1e-15 relative.  A wrong end weight (un-halved, or dropped)
+    changes the sum by O(h/T) ~ 1e-3 and fails; so does any interior weight that is not (t_{k+1}-t_{k-1})/2."""
+    gamma = 64.0
+    for n, seed in ((2, 1), (3, 2), (57, 3), (400, 4)):
+        t = _ragged_times(n, seed)
+        c0, c1 = 0.75, -0.5
+        tr = _zero_phase_trajectory(t, c0 + c1 * t, gamma)
+        _, amp = oracle_mod.points(tr, [0.0], [0.0], [0.0], return_amplitudes=True)
+        expect = -2 * gamma ** 2 * (c0 * (t[-1] - t[0]) + c1 * (t[-1] ** 2 - t[0] ** 2) / 2)
+        assert amp[0, 0].imag == 0.0
+        assert abs(amp[0, 0].real - expect) <= 1e-15 * abs(expect), (n, amp[0, 0].real, expect)
+        assert amp[0, 1] == 0 and amp[0, 2] == 0 and amp[0, 3] == 0     # ay = az = 0, n = 0
+
+
+def test_q1_rule_is_the_trapezoid_not_a_higher_order_one(oracle_mod):
+    """For a QUADRATIC integrand the composite trapezoid rule has the closed-form excess
+    sum_i h_i^3 / 6 per unit of curvature over the exact integral (interval error h^3 f''/12 with f'' = 2);
+    Simpson-type rules would be exact and a midpoint/rectangle rule has a different excess.  1e-14 relative."""
+    gamma = 64.0
+    t = _ragged_times(200, 7)
+    tr = _zero_phase_trajectory(t, t * t, gamma)
+    _, amp = oracle_mod.points(tr, [0.0], [0.0], [0.0], return_amplitudes=True)
+    h = np.diff(t)
+    expect = -2 * gamma ** 2 * ((t[-1] ** 3 - t[0] ** 3) / 3 + (h ** 3).sum() / 6)
+    assert abs(amp[0, 0].real - expect) <= 1e-14 * abs(expect)
+
+
+def test_q6_gamma_is_used_sample_wise_in_the_integrand(oracle_mod):
+    """Reading Q6, first half: 1/(2 gamma_k^2) enters eqs. (3)-(7) with the sample's own gamma_k.  With
+    gamma_k^2 linear in t and constant ax, f_x = -2 gamma_k^2 ax is linear, so the trapezoid sum is exact:
+    A_x = -2 ax [g2_0 T + s (t_N^2 - t_0^2)/2 - s t_0 T].  A single gamma (first, last or mean) for the whole
+    trajectory gives a different number at the 10 % level."""
+    t = _ragged_times(120, 11)
+    g2 = 4096.0 + 2048.0 * (t - t[0])                      # gamma^2, dyadic
+    gam = np.sqrt(g2)
+    tr = _zero_phase_trajectory(t, np.full_like(t, 0.5), gam)
+    _, amp = oracle_mod.points(tr, [0.0], [0.0], [0.0], return_amplitudes=True)
+    T = t[-1] - t[0]
+    expect = -2 * 0.5 * (4096.0 * T + 2048.0 * ((t[-1] ** 2 - t[0] ** 2) / 2 - t[0] * T))
+    # gamma_k = sqrt(g2) is rounded to double before the oracle squares it again: 2 ulp per sample
+    assert abs(amp[0, 0].real - expect) <= 1e-15 * abs(expect) * 4
+
+
+def test_q6_j_coefficient_uses_the_first_gamma(oracle_mod):
+    """Reading Q6, second half: the coefficient w^2/(2 E^2 gamma^2) of eq. (10) is taken with
+    gamma_0 = gamma[0] (E is fixed "to the value at entering the section").  On a trajectory whose
+    gamma falls by a factor 2, identity P7(iii) isolates the coefficient:
+        [spin-1/2 - (1+(1-u)^2)/(2(1-u)) spin-0] * 8 pi^2 / (u^2 |J|^2) = 1/gamma_0^2,
+    which differs by 4x from the last sample's gamma and by ~2x from the mean."""
+    wl = workloads.make("cfg3", n=3000, n_omega=6, n_th=3)
+    tr = {k: v.copy() for k, v in wl.traj.items()}
+    g0 = tr["gamma"][0]
+    tr["gamma"] = g0 * np.linspace(1.0, 0.5, len(tr["t"]))
+    lam = wl.hbarc_over_E
+    w, nx, ny = oracle_mod.grid_points(wl.omega[-3:], wl.thx, wl.thy)      # u = 0.79 ... 0.8: J term matters
+    u = w * lam
+    s0 = oracle_mod.points(tr, w, nx, ny, S0, lam)
+    sh, amp = oracle_mod.points(tr, w, nx, ny, SH, lam, return_amplitudes=True)
+    j2 = np.abs(amp[:, 3]) ** 2
+    coeff = (sh - (1 + (1 - u) ** 2) / (2 * (1 - u)) * s0) * 8 * math.pi ** 2 / (u ** 2 * j2)
+    # the difference cancels ~ S/(u^2 J^2/gamma^2) digits: keep points where the J term is not negligible
+    keep = u ** 2 * j2 / g0 ** 2 > 1e-6 * sh * 8 * math.pi ** 2
+    assert keep.sum() >= 5
+    np.testing.assert_allclose(coeff[keep], 1 / g0 ** 2, rtol=1e-8)
+    assert np.all(np.abs(coeff[keep] * tr["gamma"][-1] ** 2 - 1) > 0.5)
