@@ -608,7 +608,7 @@ static cudaError_t launch_sep(const MainParams &mp, dim3 grid, cudaStream_t st) 
                                         SepShape<NC, WY>::SMEM);
     });
     if (attr_err != cudaSuccess) return attr_err;
-    rad_sep_kernel<NC, WY><<<grid, SEP_T, SepShape<NC, WY>::SMEM, st>>>(mp);
+    rad_sep_kernel<NC, WY><<<grid, SepRegs<NC>::THREADS, SepShape<NC, WY>::SMEM, st>>>(mp);
     ++g_launches;
     return cudaGetLastError();
 }

@@ -28,8 +28,12 @@
 namespace rad {
 
 constexpr int SEP_CONS = 256;  // consumer threads
-constexpr int SEP_PROD = 128;  // producer threads
-constexpr int SEP_T = SEP_CONS + SEP_PROD;
+#ifndef RAD_SEP_PROD4
+#define RAD_SEP_PROD4 128
+#endif
+#ifndef RAD_SEP_PROD6
+#define RAD_SEP_PROD6 128
+#endif
 #ifndef RAD_SEP_S
 #define RAD_SEP_S 8
 #endif
@@ -43,20 +47,37 @@ constexpr int SEP_T = SEP_CONS + SEP_PROD;
 #define RAD_SEP_REGS_CONS4 192
 #endif
 #ifndef RAD_SEP_REGS_CONS6
-#define RAD_SEP_REGS_CONS6 200
+#define RAD_SEP_REGS_CONS6 176
+#endif
+#ifndef RAD_SEP_PU4
+#define RAD_SEP_PU4 1
+#endif
+#ifndef RAD_SEP_PU6
+#define RAD_SEP_PU6 8
 #endif
 constexpr int SEP_S = RAD_SEP_S;       // samples per table sub-block
 constexpr int SEP_NB = RAD_SEP_NB;     // table buffers in flight
 constexpr int SEP_STAGES = 3;  // trajectory-chunk ring depth
-constexpr int SEP_REGS_LAUNCH = 168;                         // __launch_bounds__(384, 1): 65536 / 384 rounded down to 8
-// setmaxnreg moves registers between the roles inside the pool the CTA got at launch (384 * 168):
-// 256 * CONS + 128 * PROD <= 384 * 168, both multiples of 8.  Measured best splits: 192 / 120 with
-// 4 accumulators per point (the producers build 6 table entries per sample and need the room),
-// 200 / 104 with 6 (the producers build 4, the consumers carry the J accumulators).
+// Producer threads per CTA (RAD_SEP_PROD4 / RAD_SEP_PROD6) and the register split.
+// setmaxnreg moves registers between the roles inside the pool the CTA got at launch
+// (THREADS * REGS_LAUNCH): 256 * CONS + NPROD * PROD <= that pool, both multiples of 8.
+// Measured (round 2, ncu source page): with 6 accumulators per point the tables serve only 8 points per
+// consumer thread and the kernel is PRODUCER-bound -- the four producer warps never wait, the consumers
+// wait for tables 17-21 % of their time.  What helped: unrolling the producers' sample loop fully
+// (RAD_SEP_PU6 = 8: 32 independent phasor chains per thread instead of 4) and moving registers to them
+// (176 / 152 instead of 200 / 104): +5.8 %.  What did not: eight producer warps with one T and one Y-or-F
+// entry per thread (RAD_SEP_PROD6 = 256, 80-96 registers each: spills, -3 ... -10 %), finer or deeper table
+// rings (4-sample sub-blocks x 4), the magic-number range reduction instead of FRND.F64 (+-0).
 template <int NC> struct SepRegs {
+    static constexpr int NPROD = NC == 6 ? RAD_SEP_PROD6 : RAD_SEP_PROD4;     // producer threads
+    static constexpr int THREADS = SEP_CONS + NPROD;
+    static constexpr int REGS_LAUNCH = 65536 / THREADS / 8 * 8;               // __launch_bounds__(THREADS, 1)
     static constexpr int CONS = NC == 6 ? RAD_SEP_REGS_CONS6 : RAD_SEP_REGS_CONS4;
-    static constexpr int PROD = ((SEP_T * SEP_REGS_LAUNCH - SEP_CONS * CONS) / SEP_PROD) / 8 * 8;
-    static_assert(CONS % 8 == 0 && PROD >= 24 && SEP_CONS * CONS + SEP_PROD * PROD <= SEP_T * SEP_REGS_LAUNCH,
+    static constexpr int PROD = ((THREADS * REGS_LAUNCH - SEP_CONS * CONS) / NPROD) / 8 * 8;
+    // samples the producers work on at once: their phasor chains are ~15 dependent FP64 steps long, and one
+    // producer warp per sub-partition has only its own instruction-level parallelism to hide that latency
+    static constexpr int PROD_UNROLL = NC == 6 ? RAD_SEP_PU6 : RAD_SEP_PU4;
+    static_assert(CONS % 8 == 0 && PROD >= 24 && SEP_CONS * CONS + NPROD * PROD <= THREADS * REGS_LAUNCH,
                   "setmaxnreg.inc would wait forever for registers the CTA does not own");
 };
 
@@ -144,8 +165,8 @@ template <int REGS> __device__ __forceinline__ void reg_alloc() {
 template <int REGS> __device__ __forceinline__ void reg_dealloc() {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REGS));
 }
-__device__ __forceinline__ void producer_bar_sync() {          // named barrier 1: the 128 producer threads
-    asm volatile("bar.sync 1, 128;" ::: "memory");
+template <int NPROD> __device__ __forceinline__ void producer_bar_sync() {   // named barrier 1: the producer threads
+    asm volatile("bar.sync 1, %0;" ::"n"(NPROD) : "memory");
 }
 
 // The sequence of (trajectory, chunk, sub-block) steps of one CTA.  Producers and consumers each run
@@ -197,7 +218,7 @@ struct SepCursor {
 
 // ------------------------------------------------------------------------------ main (a0-a7)
 template <int NC, int WY>
-__global__ void __launch_bounds__(SEP_T, 1)
+__global__ void __launch_bounds__(SepRegs<NC>::THREADS, 1)
 rad_sep_kernel(const MainParams P) {
     using SH = SepShape<NC, WY>;
     constexpr int YN = SH::YN, EV = SH::EV, S = SEP_S, NB = SEP_NB;
@@ -214,7 +235,7 @@ rad_sep_kernel(const MainParams P) {
 
     if (tid == 0) {
         for (int s = 0; s < SEP_STAGES; ++s) mbar_init(&bars[s], 1);
-        for (int b = 0; b < NB; ++b) { mbar_init(&full[b], SEP_PROD / 32); mbar_init(&empty[b], SEP_CONS / 32); }
+        for (int b = 0; b < NB; ++b) { mbar_init(&full[b], SepRegs<NC>::NPROD / 32); mbar_init(&empty[b], SEP_CONS / 32); }
         mbar_fence_init();
     }
     __syncthreads();
@@ -225,11 +246,19 @@ rad_sep_kernel(const MainParams P) {
         const int pt = tid - SEP_CONS;
         const int tile_bx = blockIdx.x;
         const SepCoord<WY> co(tile_bx, 0, P.n_thx, P.n_thy);             // tile bases only
-        constexpr int RT = 256 / SEP_PROD, RY = YN / SEP_PROD;           // entries per thread and table
+        // Entries per thread and sample.  T: 256 / NPROD.  Y and F: YN / NPROD each, or -- when there are more
+        // producer threads than Y entries -- one Y entry for threads [0, YN) and one F entry for the rest
+        // (whole warps take one role: YN is a multiple of 32).
+        constexpr int NPROD = SepRegs<NC>::NPROD;
+        constexpr bool SPLIT = YN < NPROD;
+        static_assert(256 % NPROD == 0 && (SPLIT ? 2 * YN == NPROD : YN % NPROD == 0), "producer entry assignment");
+        constexpr int RT = 256 / NPROD, RY = SPLIT ? 1 : YN / NPROD;
+        const bool doY = !SPLIT || pt < YN, doF = !SPLIT || pt >= YN;
+        const int ptF = SPLIT ? (pt >= YN ? pt - YN : 0) : pt, ptY = SPLIT ? (pt < YN ? pt : 0) : pt;
         double omT[RT], nxT[RT], omY[RY], nyY[RY], nxF[RY], nyF[RY], hF[RY];
 #pragma unroll
         for (int r = 0; r < RT; ++r) {
-            const int b = pt + r * SEP_PROD;
+            const int b = pt + r * NPROD;
             const int iw = co.bw + 4 * (b >> 6) + 2 * (b & 1) + ((b >> 4) & 1);
             const int ix = co.bx + 8 * ((b >> 5) & 1) + 2 * ((b >> 1) & 3) + ((b >> 3) & 1);
             omT[r] = P.omega[min(iw, P.n_omega - 1)];
@@ -237,8 +266,8 @@ rad_sep_kernel(const MainParams P) {
         }
 #pragma unroll
         for (int r = 0; r < RY; ++r) {
-            const int b = pt + r * SEP_PROD;
             {
+                const int b = ptY + r * NPROD;
                 const int q = b >> 3, m = q % WY, i = (q / WY) & 1, ww = (q / WY) >> 1;
                 const int iw = co.bw + 4 * ww + 2 * (b & 1) + i;
                 const int iy = co.by + WY * ((b >> 1) & 3) + m;
@@ -246,6 +275,7 @@ rad_sep_kernel(const MainParams P) {
                 nyY[r] = P.thy[min(iy, P.n_thy - 1)];
             }
             {
+                const int b = ptF + r * NPROD;
                 const int q = b >> 4, m = q % WY, j = (q / WY) & 1, wx = (q / WY) >> 1;
                 const int ix = co.bx + 8 * wx + 2 * ((b >> 2) & 3) + j;
                 const int iy = co.by + WY * (b & 3) + m;
@@ -296,6 +326,7 @@ rad_sep_kernel(const MainParams P) {
                 }
 #pragma unroll
                 for (int r = 0; r < RY; ++r) {
+                    if (!doY) continue;
                     const dd wt = omega_star_turns(omY[r], lam);
                     const dd hy = half_square_dd(nyY[r]);
                     dd psi = dd_mul_d(hy, h23.x);
@@ -309,7 +340,7 @@ rad_sep_kernel(const MainParams P) {
                 const int buf = g % NB;
                 mbar_wait(&empty[buf], ((g / NB) & 1) ^ 1);
                 const double *rec = ck + HDR + cur.sb * S * REC;
-#pragma unroll 1
+#pragma unroll SepRegs<NC>::PROD_UNROLL
                 for (int s = 0; s < S; ++s, rec += REC) {
                     const int row = buf * S + s;
                     const double2 r67 = *reinterpret_cast<const double2 *>(rec + 6);   // dP0, dt
@@ -318,14 +349,16 @@ rad_sep_kernel(const MainParams P) {
                     for (int r = 0; r < RT; ++r) {
                         const double dT = fma(-nxT[r], r89.x, fma(hxT[r], r67.y, r67.x));
                         const double2 ph = phasor_full(fma(whT[r], dT, p0T[r]));
-                        Tt[row * 256 + pt + r * SEP_PROD] = ph;
+                        Tt[row * 256 + pt + r * NPROD] = ph;
                     }
 #pragma unroll
                     for (int r = 0; r < RY; ++r) {
+                        if (!doY) continue;
                         const double dY = fma(-nyY[r], r89.y, hyY[r] * r67.y);
                         const double2 ph = phasor_full(fma(whY[r], dY, p0Y[r]));
-                        Yt[row * YN + pt + r * SEP_PROD] = ph;
+                        Yt[row * YN + ptY + r * NPROD] = ph;
                     }
+                    if (!doF) continue;
                     const double2 r01 = *reinterpret_cast<const double2 *>(rec);       // D0, vx
                     const double2 r23 = *reinterpret_cast<const double2 *>(rec + 2);   // vy, w ax
                     const double2 r45 = *reinterpret_cast<const double2 *>(rec + 4);   // w ay, w az
@@ -339,9 +372,9 @@ rad_sep_kernel(const MainParams P) {
                         const double gq = inv_square(q);
                         const double s1 = fma(nyF[r], r45.x, r45.y);
                         const double s2 = fma(nxF[r], r23.y, r45.y);
-                        Ft[row * YN + pt + r * SEP_PROD] = make_double2(fma(s1, ux, -(bx * r23.y)) * gq,
-                                                                        fma(s2, uy, -(by * r45.x)) * gq);
-                        if (NC == 6) Hh[row * YN + pt + r * SEP_PROD] = fma(nxF[r], r23.y, s1) * gq;
+                        Ft[row * YN + ptF + r * NPROD] = make_double2(fma(s1, ux, -(bx * r23.y)) * gq,
+                                                                      fma(s2, uy, -(by * r45.x)) * gq);
+                        if (NC == 6) Hh[row * YN + ptF + r * NPROD] = fma(nxF[r], r23.y, s1) * gq;
                     }
                 }
                 __syncwarp();
@@ -351,7 +384,7 @@ rad_sep_kernel(const MainParams P) {
             } while (adv == 0);
             // ---- chunk finished by every producer: its ring stage can be refilled
             ++it;
-            producer_bar_sync();
+            producer_bar_sync<NPROD>();
             if (pt == 0) produce();
         }
         return;
@@ -419,30 +452,49 @@ rad_sep_kernel(const MainParams P) {
             for (int i = 0; i < 2; ++i)
 #pragma unroll
                 for (int j = 0; j < 2; ++j) tv[i][j] = tp[(i * 2 + j) * 8];
+            // Groups g = (m, j): the two points (i = 0, 1) that share the integrand entry F[j][m].  The complex
+            // products q = T Y of group g + 1 are formed while group g is accumulated, so that every operand
+            // of the accumulation is old and the DFMAs can run in f-major order: runs that share one
+            // multiplicand in the same operand slot (register-file bandwidth: DESIGN.md 5.4 (iii)).
+            constexpr int G = 2 * WY;
+            double qr[2], qi[2];
+            auto products = [&](int g, double (&pr)[2], double (&pi)[2]) {
+                const int m = g >> 1, j = g & 1;
 #pragma unroll
-            for (int m = 0; m < WY; ++m) {
-                double2 yv[2];
+                for (int i = 0; i < 2; ++i) {
+                    const double2 y = yp[(i * WY + m) * 8];
+                    pr[i] = tv[i][j].x * y.x;
+                    pi[i] = tv[i][j].x * y.y;
+                    pr[i] = fma(-tv[i][j].y, y.y, pr[i]);
+                    pi[i] = fma(tv[i][j].y, y.x, pi[i]);
+                }
+            };
+            products(0, qr, qi);
 #pragma unroll
-                for (int i = 0; i < 2; ++i) yv[i] = yp[(i * WY + m) * 8];
+            for (int g = 0; g < G; ++g) {
+                const int m = g >> 1, j = g & 1;
+                double nr[2], ni[2];
+                if (g + 1 < G) products(g + 1, nr, ni);
+                const double2 f = fp[(j * WY + m) * 16];
+                double *a0 = acc[(0 * 2 + j) * WY + m], *a1 = acc[(1 * 2 + j) * WY + m];
+                a0[0] = fma(f.x, qr[0], a0[0]);
+                a0[1] = fma(f.x, qi[0], a0[1]);
+                a1[0] = fma(f.x, qr[1], a1[0]);
+                a1[1] = fma(f.x, qi[1], a1[1]);
+                a1[3] = fma(f.y, qi[1], a1[3]);
+                a1[2] = fma(f.y, qr[1], a1[2]);
+                a0[3] = fma(f.y, qi[0], a0[3]);
+                a0[2] = fma(f.y, qr[0], a0[2]);
+                if (NC == 6) {
+                    const double hv = hp[(j * WY + m) * 16];
+                    a0[4] = fma(hv, qr[0], a0[4]);
+                    a0[5] = fma(hv, qi[0], a0[5]);
+                    a1[4] = fma(hv, qr[1], a1[4]);
+                    a1[5] = fma(hv, qi[1], a1[5]);
+                }
+                if (g + 1 < G) {
 #pragma unroll
-                for (int j = 0; j < 2; ++j) {
-                    const double2 f = fp[(j * WY + m) * 16];
-                    double hv = 0.0;
-                    if (NC == 6) hv = hp[(j * WY + m) * 16];
-#pragma unroll
-                    for (int i = 0; i < 2; ++i) {
-                        const double qr = fma(-tv[i][j].y, yv[i].y, tv[i][j].x * yv[i].x);
-                        const double qi = fma(tv[i][j].y, yv[i].x, tv[i][j].x * yv[i].y);
-                        double *a = acc[(i * 2 + j) * WY + m];
-                        a[0] = fma(f.x, qr, a[0]);
-                        a[1] = fma(f.x, qi, a[1]);
-                        a[2] = fma(f.y, qr, a[2]);
-                        a[3] = fma(f.y, qi, a[3]);
-                        if (NC == 6) {
-                            a[4] = fma(hv, qr, a[4]);
-                            a[5] = fma(hv, qi, a[5]);
-                        }
-                    }
+                    for (int i = 0; i < 2; ++i) { qr[i] = nr[i]; qi[i] = ni[i]; }
                 }
             }
         }
