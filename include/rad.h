@@ -45,6 +45,8 @@
  *     samples.  A grid point with u = omega * hbarc_over_E >= 1 (photon energy above
  *     the particle energy, no final state) yields NaN at that point (the omega array
  *     lives on the device; no host-side check, no sync).
+ *   - `opt` (last argument but one of every compute call) carries per-call options; NULL = defaults.
+ *     There is no process-wide switch: two threads may call with different options.
  *   - Results are deterministic run to run (fixed reduction order, no FP atomics).
  *   - There is no CPU fallback: without a CUDA device every compute call returns
  *     RAD_ECUDA.
@@ -68,6 +70,40 @@ typedef enum {
 } rad_status;
 
 typedef enum { RAD_CLASSICAL = 0, RAD_SPIN0 = 1, RAD_SPIN_HALF = 2 } rad_model;
+
+/* Which main kernel evaluates the integrals.
+ *   RAD_KERNEL_AUTO       chosen from the shapes (what every shipped workload uses):
+ *                         - the separable-phasor kernel (e^{i w psi} = T(w, n_x) Y(w, n_y) on a tensor grid, exact
+ *                           because theta^2 = n_x^2 + n_y^2, eq. (7)) on the part of the grid that
+ *                           fills its 16 x 16 x 16 (spin-1/2: 16 x 16 x 8) point tiles; angle rows / columns left
+ *                           over (e.g. the paper's typical 50 x 50 angles: 48 x 48 + an L-shaped
+ *                           rest) go to the direct kernel in a second launch when that is cheaper than padding;
+ *                         - the direct kernel (one phasor per eval) where the grid fills those tiles badly;
+ *                         - the fused single-launch kernel for one short trajectory on a grid too small to fill
+ *                           the GPU (a cooperative launch: pack, time split over all SMs, grid-wide ordered
+ *                           reduction and epilogue in one kernel).
+ *   RAD_KERNEL_DIRECT     always the direct kernel (separate pack / main / reduction launches)
+ *   RAD_KERNEL_SEPARABLE  always the separable kernel, padding the grid to whole tiles
+ *   RAD_KERNEL_FUSED      the fused single-launch kernel; RAD_EINVAL where it does not apply (count > 1,
+ *                         more tiles than fit on the GPU at once)
+ * All of them meet the same tolerance and are parity-tested separately. */
+typedef enum { RAD_KERNEL_AUTO = 0, RAD_KERNEL_DIRECT = 1, RAD_KERNEL_SEPARABLE = 2, RAD_KERNEL_FUSED = 3 } rad_kernel;
+
+/* Per-kernel timing of ONE call (bench.py's roofline needs the main kernel's own duration): an opaque set of
+ * CUDA events created on the current device.  Pass it in rad_options.profile; the call records the events on
+ * its stream around its pack / main / reduction launches; rad_profile_read waits for the last one and returns
+ * ms[0..2] = pack, main (all main-kernel launches of the call), reduction durations (0 where not run).
+ * One profile object must not be used by two calls at the same time. */
+typedef struct rad_profile rad_profile;
+rad_profile *rad_profile_create(void);                 /* NULL on failure (no device) */
+void rad_profile_destroy(rad_profile *profile);
+int rad_profile_read(rad_profile *profile, float *ms);
+
+typedef struct {
+    int32_t kernel;          /* rad_kernel; 0 = auto */
+    int32_t reserved;        /* must be 0 */
+    rad_profile *profile;    /* NULL: no timing */
+} rad_options;
 
 /* One trajectory (or one crystal section), structure of arrays, n >= 2 samples.
  * t: time; dz = z - beta0 t; x, y; vx, vy; dvz = v_z - beta0 (beta0 = 1 - 1/2gamma^2,
@@ -96,46 +132,67 @@ typedef struct {
 
 /* Classical spectrum, eq. (1) with eqs. (3)-(7).  out: n_omega*n_thy*n_thx doubles. */
 int rad_classical(const rad_traj *traj, const rad_grid *grid, double *out,
-                  void *workspace, size_t workspace_bytes, void *cuda_stream);
+                  void *workspace, size_t workspace_bytes, const rad_options *opt, void *cuda_stream);
 
 /* Semi-classical spectrum.  spin = 0: substitution model, eq. (9); spin = 1: spin-1/2,
  * BCK eq. (10).  hbarc_over_E = hbar c / E in the length unit, so that
  * u = hbar w / E = omega * hbarc_over_E and w* = omega / (1 - u). */
 int rad_semiclassical(const rad_traj *traj, const rad_grid *grid, int spin,
                       double hbarc_over_E, double *out,
-                      void *workspace, size_t workspace_bytes, void *cuda_stream);
+                      void *workspace, size_t workspace_bytes, const rad_options *opt, void *cuda_stream);
 
 /* out[m] (+)= sum over p (ascending) of the spectrum of trajectory p.
  * hbarc_over_E: HOST array, one per trajectory (NULL allowed iff model is classical).
  * accumulate: 0 overwrites out, 1 adds to it (resume a partial ensemble). */
 int rad_ensemble_sum(const rad_traj_batch *batch, const rad_grid *grid, rad_model model,
                      const double *hbarc_over_E, int accumulate, double *out,
-                     void *workspace, size_t workspace_bytes, void *cuda_stream);
+                     void *workspace, size_t workspace_bytes, const rad_options *opt, void *cuda_stream);
 
-/* dI/dw of an ensemble WITHOUT materialising the whole cube (3000^2 angles x 100 omegas
- * "approach the limit" of GPU memory at one double per integral): the grid is processed in slabs of omegas
- * whose cube (<= ~256 MB) lives in the workspace, each slab summed over the angles as rad_angular_sum does.
+/* dI/dw[i_w] = d_solid_angle * sum over the angles of the spectrum of an ensemble, optionally only where
+ * n_x^2 + n_y^2 <= theta_cut^2 (theta_cut <= 0: no mask) -- the paper's "final sum over the spatial integrals"
+ * -- WITHOUT the cube (3000^2 angles x 100 omegas "approach the limit" of GPU
+ * memory at one double per integral).  When the grid fills the GPU (one CTA per tile, no time / trajectory
+ * split) the sum over a tile's angles is formed in the main kernel's epilogue in a fixed order, one partial per
+ * (tile, omega) is written and a small second pass adds the partials in tile order: no cube is written at all.
+ * Smaller grids (fewer than 8 tiles per SM: their cube is < 40 MB) are evaluated into a cube inside the
+ * workspace and summed by rad_angular_sum.
  * spectrum: n_omega doubles (device), overwritten.  workspace: DEVICE, 256-byte aligned, REQUIRED here, at
  * least rad_angular_spectrum_workspace_bytes() bytes.  batch->n and hbarc_over_E are HOST arrays as in
  * rad_ensemble_sum (count = 1 for a single trajectory).  Same values as cube + rad_angular_sum up to the
- * rounding of a different time / trajectory split (a slab has its own launch plan). */
+ * rounding of a different summation order. */
 int rad_angular_spectrum(const rad_traj_batch *batch, const rad_grid *grid, rad_model model,
                          const double *hbarc_over_E, double d_solid_angle, double theta_cut, double *spectrum,
-                         void *workspace, size_t workspace_bytes, void *cuda_stream);
+                         void *workspace, size_t workspace_bytes, const rad_options *opt, void *cuda_stream);
 size_t rad_angular_spectrum_workspace_bytes(int32_t count, int64_t n_max, int32_t n_omega, int32_t n_thx,
                                             int32_t n_thy);
+
+/* Photon NUMBER spectrum from an intensity spectrum (eqs. 8-9: the substitution model is
+ * stated for dN/d(hbar w); dI = hbar w dN):  number[i] = spectrum[i] / (hbar_c * omega[i]), i.e. with
+ * spectrum = dI/dw (per rad/length, as rad_angular_spectrum returns it) and hbar_c in energy x length this is
+ * dN/dw = (dI/dw) / (hbar w); divide by hbar_c once more for dN/d(hbar w).  omega[i] = 0 gives +inf (or NaN for
+ * 0/0), as the formula does.  All arrays DEVICE, n entries; number may alias spectrum. */
+int rad_number_spectrum(const double *spectrum, const double *omega, int32_t n, double hbar_c, double *number,
+                        void *cuda_stream);
 
 /* One long trajectory cut into sections with their own energy -- the paper's treatment of energy
  * loss: "the total spectrum is then the sum of the spectra from each section".
  * out[m] (+)= sum over s (ascending) of the spectrum of samples start[s] .. start[s+1], BOTH included:
  * neighbouring sections share their boundary sample, so their trapezoid weights tile the time axis.
  * start: HOST array of n_sections + 1 strictly ascending sample indices in [0, traj->n - 1];
- * hbarc_over_E: HOST array, one per section (NULL allowed iff classical); the J coefficient of
- * eq. (10) uses gamma of each section's first sample.  Choosing the sections (each longer than the
- * formation length l_f = 2 gamma^2 (E - w)/(E w)) is the caller's business: not checked. */
+ * hbarc_over_E: HOST array, one per section (NULL allowed iff classical).
+ * Boundary-sample rule: sample start[s] (s > 0) belongs to sections s - 1 and s and is read from the ONE array
+ * entry both times -- gamma[start[s]] enters 1/(2 gamma_k^2) of both sections' end weights, and the J
+ * coefficient of eq. (10) of section s uses gamma[start[s]] (its first sample).  A caller who fixes E per
+ * section "to the value at entering the section" therefore stores the NEW section's gamma at the
+ * boundary sample; the energies differ by the loss over one section, which is the approximation the paper
+ * makes anyway.  Sections with exactly their own arrays are what rad_ensemble_sum takes.
+ * Choosing the sections (each longer than the formation length) is the caller's business; this
+ * call does not check it -- rad_sections_check does, on host-visible numbers.
+ * start and hbarc_over_E are read before the call returns (copied to the device through the stream; pageable
+ * memory is staged by the runtime, pinned memory must stay valid until the stream has passed the copy). */
 int rad_sections_sum(const rad_traj *traj, int32_t n_sections, const int64_t *start, const rad_grid *grid,
                      rad_model model, const double *hbarc_over_E, int accumulate, double *out,
-                     void *workspace, size_t workspace_bytes, void *cuda_stream);
+                     void *workspace, size_t workspace_bytes, const rad_options *opt, void *cuda_stream);
 
 /* Formation length l_f = 2 gamma^2 (E - w)/(E w), in the length unit of omega (c = hbar = 1:
  * omega in rad/length, u = omega * hbarc_over_E = hbar w / E).  A section handed to rad_sections_sum must be
@@ -143,6 +200,17 @@ int rad_sections_sum(const rad_traj *traj, int32_t n_sections, const int64_t *st
  * Note: for the paper's own example (50 GeV positron, 5 GeV photon) the formula gives 680 nm, while the
  * paper prints 71 nm -- the text is at odds with itself there; the formula is what this returns. */
 double rad_formation_length(double gamma, double omega, double hbarc_over_E);
+
+/* The check PAPER.md:73-75 asks of a sectioning ("section length longer than the formation length"), on HOST
+ * arrays: section s spans t_start[s] .. t_start[s+1] (the times of the boundary samples, n_sections + 1
+ * entries, ascending; c = 1 so a time is a length), has Lorentz factor gamma0[s] and hbarc_over_E[s] (NULL:
+ * classical, u = 0).  The formation length is longest at the lowest frequency, so omega_min = the smallest
+ * POSITIVE omega of the grid decides.  Writes to `short_sections` (capacity `cap`, may be NULL if cap = 0) the
+ * indices of the sections with t_start[s+1] - t_start[s] <= l_f(gamma0[s], omega_min, hbarc_over_E[s]), in
+ * ascending order, and returns how many there are (possibly more than cap); RAD_EINVAL / RAD_EDOMAIN
+ * (negative) on bad arguments.  Host arithmetic only. */
+int rad_sections_check(int32_t n_sections, const double *t_start, const double *gamma0,
+                       const double *hbarc_over_E, double omega_min, int32_t *short_sections, int32_t cap);
 
 /* dI/dw[i_w] = sum_{i_x,i_y} cube * d_omega_solid, optionally only where
  * n_x^2 + n_y^2 <= theta_cut^2 (theta_cut <= 0: no mask) -- the paper's "final sum over
@@ -194,47 +262,37 @@ size_t rad_workspace_bytes(int32_t count, int64_t n_max,
 /* HOST-buffer variants (the paper's flow: trajectory copied to the GPU once, cube copied
  * back once).  Every pointer inside traj/batch/grid and `out` is HOST memory
  * (pinned memory makes the copies asynchronous).  Device buffers come from the
- * stream-ordered pool; the call returns after the result is in `out`.
+ * stream-ordered pool; the call returns after the result is in `out` (it synchronises the stream once).
  * model: rad_model; hbarc_over_E ignored for RAD_CLASSICAL. */
 int rad_eval_host(const rad_traj *traj, const rad_grid *grid, rad_model model,
-                  double hbarc_over_E, double *out, void *cuda_stream);
+                  double hbarc_over_E, double *out, const rad_options *opt, void *cuda_stream);
 int rad_ensemble_sum_host(const rad_traj_batch *batch, const rad_grid *grid, rad_model model,
                           const double *hbarc_over_E, int accumulate, double *out,
-                          void *cuda_stream);
+                          const rad_options *opt, void *cuda_stream);
 
 /* FP64 FMA peak of the current device, measured: runs a register-resident DFMA chain
  * kernel for about `millis` ms and returns FLOP/s (2 per FMA lane); <= 0 on error. */
 double rad_measure_fp64_peak(double millis, void *cuda_stream);
 
-/* Number of kernels the library has launched in this process (bench bookkeeping). */
+/* Number of kernels the library has launched in this process (bench bookkeeping; a relaxed atomic counter,
+ * the only process-wide state besides per-device attribute caches). */
 int64_t rad_launch_count(void);
 
-/* Which main kernel later calls use.  0 (default): chosen from the grid shape -- the separable-phasor
- * kernel (e^{i w psi} = T(w, n_x) Y(w, n_y) on a tensor grid, exact because theta^2 = n_x^2 + n_y^2,
- * eq. (7)) when the grid fills at least 60 % (spin-1/2: 75 %) of its 16 x 16 x 16 (spin-1/2:
- * 16 x 16 x 8) point tiles after padding, else the direct kernel (one phasor per eval).  1: always direct,
- * 2: always separable.  Both meet the same tolerance; process-wide; RAD_EINVAL on other values. */
-int rad_set_kernel(int choice);
+/* Which kernel a call on a grid of this shape uses for `count` trajectories of at most n_max samples under
+ * the option `kernel` (a rad_kernel): 1 direct, 2 separable, 3 fused -- for the largest part of the grid when the
+ * call is split in two launches.  A pure function of the arguments and the SM count (148 assumed when no device
+ * is visible); RAD_EINVAL on bad input. */
+int rad_plan_kernel(int32_t count, int64_t n_max, int32_t n_omega, int32_t n_thx, int32_t n_thy,
+                    rad_model model, int32_t kernel);
 
-/* Which kernel a call on a grid of this shape uses under the current rad_set_kernel setting:
- * 1 direct, 2 separable (a pure function of the arguments; no device needed); RAD_EINVAL on bad input. */
-int rad_plan_kernel(int32_t n_omega, int32_t n_thx, int32_t n_thy, rad_model model);
-
-/* The launch plan of a call of this shape (a pure function of the arguments, the rad_set_kernel setting and
- * the SM count; 148 SMs assumed when no device is visible): plan[0] kernel (1 direct, 2 separable),
- * plan[1] mode (0 one CTA per tile, 1 trajectory axis sliced, 2 time axis sliced), plan[2] tiles =
- * gridDim.x, plan[3] slices = gridDim.y, plan[4] time slices per trajectory, plan[5] chunks of 128
- * samples per trajectory.  For inspection and tests. */
+/* The launch plan of such a call, for inspection and tests: plan[0] kernel of the first (largest) part (1 direct,
+ * 2 separable, 3 fused), plan[1] its mode (0 one CTA per tile, 1 trajectory axis sliced, 2 time axis sliced),
+ * plan[2] tiles = gridDim.x, plan[3] slices = gridDim.y, plan[4] time slices per trajectory, plan[5] chunks of
+ * 128 samples per trajectory, plan[6] number of parts (2: separable interior + direct kernel on the L-shaped
+ * rest of the angle plane), plan[7] angle columns and plan[8] angle rows of the separable interior (0 if none),
+ * plan[9] kernel launches of the whole call. */
 int rad_plan_describe(int32_t count, int64_t n_max, int32_t n_omega, int32_t n_thx, int32_t n_thy,
-                      rad_model model, int32_t *plan);
-
-/* Per-kernel timing of the most recent device-buffer call (for the roofline in bench.py).
- * rad_profile_enable(1) makes every later call record CUDA events on its stream around the
- * pack, main and finalize kernels; rad_profile_last waits for that call's last event and
- * writes ms[0..2] = pack, main, finalize durations in milliseconds (finalize 0 if not run).
- * Not thread-safe across concurrent calls; off by default. */
-int rad_profile_enable(int on);
-int rad_profile_last(float *ms);
+                      rad_model model, int32_t kernel, int32_t *plan);
 
 /* Static text for a rad_status; for RAD_ECUDA the text of the last CUDA error seen. */
 const char *rad_strerror(int code);

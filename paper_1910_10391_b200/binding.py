@@ -19,9 +19,12 @@ FIELDS = ("t", "dz", "x", "y", "vx", "vy", "dvz", "ax", "ay", "az", "gamma")
 EXPORTS = ("rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_sections_sum", "rad_angular_sum", "rad_sum_cubes",
            "rad_workspace_bytes", "rad_eval_host", "rad_ensemble_sum_host",
            "rad_measure_fp64_peak", "rad_launch_count", "rad_strerror",
-           "rad_profile_enable", "rad_profile_last", "rad_set_kernel", "rad_plan_kernel",
+           "rad_profile_create", "rad_profile_destroy", "rad_profile_read", "rad_plan_kernel",
            "rad_generate_trajectories", "rad_plan_describe", "rad_angular_spectrum",
-           "rad_angular_spectrum_workspace_bytes", "rad_formation_length")
+           "rad_angular_spectrum_workspace_bytes", "rad_formation_length", "rad_sections_check",
+           "rad_number_spectrum")
+
+KERNEL_AUTO, KERNEL_DIRECT, KERNEL_SEPARABLE, KERNEL_FUSED = 0, 1, 2, 3
 
 _dp = ctypes.POINTER(ctypes.c_double)
 _lib = None
@@ -46,6 +49,10 @@ class _TrajBuffers(ctypes.Structure):
     _fields_ = [(k, ctypes.c_void_p) for k in FIELDS]
 
 
+class _Options(ctypes.Structure):
+    _fields_ = [("kernel", ctypes.c_int32), ("reserved", ctypes.c_int32), ("profile", ctypes.c_void_p)]
+
+
 class _Grid(ctypes.Structure):
     _fields_ = [("n_omega", ctypes.c_int32), ("n_thx", ctypes.c_int32), ("n_thy", ctypes.c_int32),
                 ("omega", ctypes.c_void_p), ("thx", ctypes.c_void_p), ("thy", ctypes.c_void_p)]
@@ -59,7 +66,7 @@ def build_library(force: bool = False, verbose: bool = False) -> Path:
     """Compile csrc/rad.cu for sm_100a into the in-tree shared library (nvcc cross-compiles
     without a GPU)."""
     srcs = [_SRC / "rad.cu", _SRC / "rad_device.cuh", _SRC / "rad_sep.cuh", _SRC / "rad_traj.cuh",
-            _SRC / "sincos_coeffs.h",
+            _SRC / "rad_fused.cuh", _SRC / "rad_plan.h", _SRC / "sincos_coeffs.h",
             _PKG.parent / "include" / "rad.h"]
     if not force and _SO.exists() and all(_SO.stat().st_mtime >= s.stat().st_mtime for s in srcs):
         return _SO
@@ -83,49 +90,39 @@ def load_library() -> ctypes.CDLL:
             f"{_SO} is missing: run __graft_entry__.build() (nvcc) first; there is no CPU fallback")
     lib = ctypes.CDLL(str(_SO))
     vp, sz, i32, i64, dbl = ctypes.c_void_p, ctypes.c_size_t, ctypes.c_int32, ctypes.c_int64, ctypes.c_double
-    lib.rad_classical.argtypes = [ctypes.POINTER(_Traj), ctypes.POINTER(_Grid), vp, vp, sz, vp]
-    lib.rad_semiclassical.argtypes = [ctypes.POINTER(_Traj), ctypes.POINTER(_Grid), ctypes.c_int, dbl,
-                                      vp, vp, sz, vp]
-    lib.rad_ensemble_sum.argtypes = [ctypes.POINTER(_Batch), ctypes.POINTER(_Grid), ctypes.c_int, vp,
-                                     ctypes.c_int, vp, vp, sz, vp]
-    lib.rad_sections_sum.argtypes = [ctypes.POINTER(_Traj), i32, vp, ctypes.POINTER(_Grid), ctypes.c_int, vp,
-                                     ctypes.c_int, vp, vp, sz, vp]
-    lib.rad_sections_sum.restype = ctypes.c_int
-    lib.rad_angular_sum.argtypes = [vp, ctypes.POINTER(_Grid), dbl, dbl, vp, vp]
-    lib.rad_sum_cubes.argtypes = [vp, i32, i64, ctypes.c_int, vp, vp]
-    lib.rad_set_kernel.argtypes = [ctypes.c_int]
-    lib.rad_set_kernel.restype = ctypes.c_int
-    lib.rad_plan_kernel.argtypes = [i32, i32, i32, ctypes.c_int]
-    lib.rad_plan_kernel.restype = ctypes.c_int
-    lib.rad_angular_spectrum.argtypes = [ctypes.POINTER(_Batch), ctypes.POINTER(_Grid), ctypes.c_int, vp, dbl, dbl,
-                                         vp, vp, sz, vp]
-    lib.rad_angular_spectrum.restype = ctypes.c_int
-    lib.rad_angular_spectrum_workspace_bytes.argtypes = [i32, i64, i32, i32, i32]
-    lib.rad_angular_spectrum_workspace_bytes.restype = sz
-    lib.rad_formation_length.argtypes = [dbl, dbl, dbl]
-    lib.rad_formation_length.restype = dbl
-    lib.rad_plan_describe.argtypes = [i32, i64, i32, i32, i32, ctypes.c_int, ctypes.POINTER(ctypes.c_int32)]
-    lib.rad_plan_describe.restype = ctypes.c_int
-    lib.rad_generate_trajectories.argtypes = ([ctypes.c_int] + [dbl] * 5 + [ctypes.c_uint64, i32, i64, i64] + [vp] * 4
-                                              + [ctypes.POINTER(_TrajBuffers), vp])
-    lib.rad_generate_trajectories.restype = ctypes.c_int
-    lib.rad_workspace_bytes.argtypes = [i32, i64, i32, i32, i32]
-    lib.rad_workspace_bytes.restype = sz
-    lib.rad_eval_host.argtypes = [ctypes.POINTER(_Traj), ctypes.POINTER(_Grid), ctypes.c_int, dbl, vp, vp]
-    lib.rad_ensemble_sum_host.argtypes = [ctypes.POINTER(_Batch), ctypes.POINTER(_Grid), ctypes.c_int, vp,
-                                          ctypes.c_int, vp, vp]
-    lib.rad_measure_fp64_peak.argtypes = [dbl, vp]
-    lib.rad_measure_fp64_peak.restype = dbl
-    lib.rad_launch_count.restype = i64
-    lib.rad_profile_enable.argtypes = [ctypes.c_int]
-    lib.rad_profile_enable.restype = ctypes.c_int
-    lib.rad_profile_last.argtypes = [ctypes.POINTER(ctypes.c_float)]
-    lib.rad_profile_last.restype = ctypes.c_int
-    lib.rad_strerror.argtypes = [ctypes.c_int]
-    lib.rad_strerror.restype = ctypes.c_char_p
-    for name in ("rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_angular_sum",
-                 "rad_sum_cubes", "rad_eval_host", "rad_ensemble_sum_host"):
-        getattr(lib, name).restype = ctypes.c_int
+    P = ctypes.POINTER
+    op = P(_Options)
+    sig = {
+        "rad_classical": (ctypes.c_int, [P(_Traj), P(_Grid), vp, vp, sz, op, vp]),
+        "rad_semiclassical": (ctypes.c_int, [P(_Traj), P(_Grid), ctypes.c_int, dbl, vp, vp, sz, op, vp]),
+        "rad_ensemble_sum": (ctypes.c_int, [P(_Batch), P(_Grid), ctypes.c_int, vp, ctypes.c_int, vp, vp, sz, op, vp]),
+        "rad_sections_sum": (ctypes.c_int, [P(_Traj), i32, vp, P(_Grid), ctypes.c_int, vp, ctypes.c_int, vp, vp, sz,
+                                            op, vp]),
+        "rad_sections_check": (ctypes.c_int, [i32, vp, vp, vp, dbl, vp, i32]),
+        "rad_angular_sum": (ctypes.c_int, [vp, P(_Grid), dbl, dbl, vp, vp]),
+        "rad_angular_spectrum": (ctypes.c_int, [P(_Batch), P(_Grid), ctypes.c_int, vp, dbl, dbl, vp, vp, sz, op, vp]),
+        "rad_angular_spectrum_workspace_bytes": (sz, [i32, i64, i32, i32, i32]),
+        "rad_number_spectrum": (ctypes.c_int, [vp, vp, i32, dbl, vp, vp]),
+        "rad_sum_cubes": (ctypes.c_int, [vp, i32, i64, ctypes.c_int, vp, vp]),
+        "rad_plan_kernel": (ctypes.c_int, [i32, i64, i32, i32, i32, ctypes.c_int, i32]),
+        "rad_plan_describe": (ctypes.c_int, [i32, i64, i32, i32, i32, ctypes.c_int, i32, P(ctypes.c_int32)]),
+        "rad_formation_length": (dbl, [dbl, dbl, dbl]),
+        "rad_generate_trajectories": (ctypes.c_int, [ctypes.c_int] + [dbl] * 5 + [ctypes.c_uint64, i32, i64, i64]
+                                      + [vp] * 4 + [P(_TrajBuffers), vp]),
+        "rad_workspace_bytes": (sz, [i32, i64, i32, i32, i32]),
+        "rad_eval_host": (ctypes.c_int, [P(_Traj), P(_Grid), ctypes.c_int, dbl, vp, op, vp]),
+        "rad_ensemble_sum_host": (ctypes.c_int, [P(_Batch), P(_Grid), ctypes.c_int, vp, ctypes.c_int, vp, op, vp]),
+        "rad_measure_fp64_peak": (dbl, [dbl, vp]),
+        "rad_launch_count": (i64, []),
+        "rad_profile_create": (vp, []),
+        "rad_profile_destroy": (None, [vp]),
+        "rad_profile_read": (ctypes.c_int, [vp, P(ctypes.c_float)]),
+        "rad_strerror": (ctypes.c_char_p, [ctypes.c_int]),
+    }
+    assert set(sig) == set(EXPORTS)
+    for name, (res, args) in sig.items():
+        fn = getattr(lib, name)
+        fn.restype, fn.argtypes = res, args
     _lib = lib
     return lib
 
@@ -161,6 +158,39 @@ def _traj_struct(traj: dict) -> _Traj:
     return _Traj(n, *[t.data_ptr() for t in ts])
 
 
+class RadProfile:
+    """Per-kernel timing of one call (include/rad.h rad_profile): pass as ``profile=`` to a compute call, then
+    ``read()`` -> (pack_ms, main_ms, reduction_ms).  Owns CUDA events of the current device."""
+
+    def __init__(self):
+        self._h = load_library().rad_profile_create()
+        if not self._h:
+            raise RadError(-3, "rad_profile_create failed (no CUDA device?)")
+
+    def read(self):
+        ms = (ctypes.c_float * 3)()
+        _check(load_library().rad_profile_read(self._h, ms))
+        return float(ms[0]), float(ms[1]), float(ms[2])
+
+    def close(self):
+        if self._h:
+            load_library().rad_profile_destroy(self._h)
+            self._h = None
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+
+def _opt(kernel: int, profile):
+    """rad_options for a call (NULL when everything is default)."""
+    if not kernel and profile is None:
+        return None
+    return ctypes.byref(_Options(int(kernel), 0, profile._h if profile is not None else None))
+
+
 def _ws_args(workspace):
     if workspace is None:
         return None, 0
@@ -183,31 +213,32 @@ def rad_workspace_bytes(count: int, n_max: int, n_omega: int, n_thx: int, n_thy:
     return int(load_library().rad_workspace_bytes(count, n_max, n_omega, n_thx, n_thy))
 
 
-def rad_classical(traj: dict, omega, thx, thy, out=None, workspace=None, stream=None):
+def rad_classical(traj: dict, omega, thx, thy, out=None, workspace=None, stream=None, kernel: int = 0, profile=None):
     """Classical cube (n_omega, n_thy, n_thx); eq. (1) with eqs. (3)-(7)."""
     g = _grid_struct(_dev(omega, "omega"), _dev(thx, "thx"), _dev(thy, "thy"))
     t = _traj_struct(traj)
     out = _out_cube(out, omega, thx, thy)
     ws, nb = _ws_args(workspace)
     _check(load_library().rad_classical(ctypes.byref(t), ctypes.byref(g), out.data_ptr(), ws, nb,
-                                        _stream_ptr(stream)))
+                                        _opt(kernel, profile), _stream_ptr(stream)))
     return out
 
 
 def rad_semiclassical(traj: dict, omega, thx, thy, spin: int, hbarc_over_E: float, out=None,
-                      workspace=None, stream=None):
+                      workspace=None, stream=None, kernel: int = 0, profile=None):
     """spin=0: substitution model, eq. (9); spin=1: spin-1/2 BCK, eq. (10) PAPER.md:62."""
     g = _grid_struct(_dev(omega, "omega"), _dev(thx, "thx"), _dev(thy, "thy"))
     t = _traj_struct(traj)
     out = _out_cube(out, omega, thx, thy)
     ws, nb = _ws_args(workspace)
     _check(load_library().rad_semiclassical(ctypes.byref(t), ctypes.byref(g), int(spin), float(hbarc_over_E),
-                                            out.data_ptr(), ws, nb, _stream_ptr(stream)))
+                                            out.data_ptr(), ws, nb, _opt(kernel, profile), _stream_ptr(stream)))
     return out
 
 
 def rad_ensemble_sum(batch: dict, n, omega, thx, thy, model: int = CLASSICAL, hbarc_over_E=None,
-                     accumulate: bool = False, out=None, workspace=None, stream=None):
+                     accumulate: bool = False, out=None, workspace=None, stream=None, kernel: int = 0,
+                     profile=None):
     """Sum of the spectra of `count` trajectories.  batch: FIELDS -> (count, stride)
     CUDA tensors; n: host int64 (count,)."""
     ts = [_dev(batch[k], k) for k in FIELDS]
@@ -229,12 +260,13 @@ def rad_ensemble_sum(batch: dict, n, omega, thx, thy, model: int = CLASSICAL, hb
     _check(load_library().rad_ensemble_sum(ctypes.byref(b), ctypes.byref(g), int(model),
                                            lam.ctypes.data if lam is not None else None,
                                            1 if accumulate else 0, out.data_ptr(), ws, nb,
-                                           _stream_ptr(stream)))
+                                           _opt(kernel, profile), _stream_ptr(stream)))
     return out
 
 
 def rad_sections_sum(traj: dict, start, omega, thx, thy, model: int = CLASSICAL, hbarc_over_E=None,
-                     accumulate: bool = False, out=None, workspace=None, stream=None):
+                     accumulate: bool = False, out=None, workspace=None, stream=None, kernel: int = 0,
+                     profile=None):
     """Sum of the spectra of the sections start[s]..start[s+1] (both included) of one trajectory, each with
     its own hbar c / E."""
     t = _traj_struct(traj)
@@ -251,7 +283,39 @@ def rad_sections_sum(traj: dict, start, omega, thx, thy, model: int = CLASSICAL,
     ws, nb = _ws_args(workspace)
     _check(load_library().rad_sections_sum(ctypes.byref(t), st.size - 1, st.ctypes.data, ctypes.byref(g), int(model),
                                            lam.ctypes.data if lam is not None else None,
-                                           1 if accumulate else 0, out.data_ptr(), ws, nb, _stream_ptr(stream)))
+                                           1 if accumulate else 0, out.data_ptr(), ws, nb, _opt(kernel, profile),
+                                           _stream_ptr(stream)))
+    return out
+
+
+def rad_sections_check(t_start, gamma0, omega_min: float, hbarc_over_E=None):
+    """Indices of the sections not longer than the formation length at omega_min.  Host arrays:
+    t_start (n_sections + 1 boundary times), gamma0 and hbarc_over_E (n_sections each; None: classical)."""
+    t = np.ascontiguousarray(t_start, dtype=np.float64)
+    g = np.ascontiguousarray(gamma0, dtype=np.float64)
+    ns = g.size
+    if t.shape != (ns + 1,):
+        raise ValueError("t_start needs n_sections + 1 entries")
+    lam = None
+    if hbarc_over_E is not None:
+        lam = np.ascontiguousarray(np.broadcast_to(np.asarray(hbarc_over_E, dtype=np.float64), (ns,)))
+    idx = np.empty(ns, dtype=np.int32)
+    rc = load_library().rad_sections_check(ns, t.ctypes.data, g.ctypes.data, lam.ctypes.data if lam is not None else None,
+                                           float(omega_min), idx.ctypes.data, ns)
+    if rc < 0:
+        _check(rc)
+    return idx[:rc].copy()
+
+
+def rad_number_spectrum(spectrum, omega, hbar_c: float, out=None, stream=None):
+    """dN/dw = (dI/dw) / (hbar_c * omega) (PAPER.md:50-56)."""
+    _dev(spectrum, "spectrum"), _dev(omega, "omega")
+    if spectrum.numel() != omega.numel():
+        raise ValueError("spectrum and omega must have one length")
+    if out is None:
+        out = torch.empty_like(spectrum)
+    _check(load_library().rad_number_spectrum(spectrum.data_ptr(), omega.data_ptr(), omega.numel(), float(hbar_c),
+                                              _dev(out, "out").data_ptr(), _stream_ptr(stream)))
     return out
 
 
@@ -309,10 +373,13 @@ def rad_sum_cubes(cubes, accumulate: bool = False, out=None, stream=None):
 
 
 def rad_angular_spectrum(batch: dict, n, omega, thx, thy, d_solid_angle: float, theta_cut: float = 0.0,
-                         model: int = CLASSICAL, hbarc_over_E=None, out=None, workspace=None, stream=None):
+                         model: int = CLASSICAL, hbarc_over_E=None, out=None, workspace=None, stream=None,
+                         kernel: int = 0, profile=None):
     """dI/dw of an ensemble, slab by slab, without the whole cube in memory."""
     ts = [_dev(batch[k], k) for k in FIELDS]
     count, stride = ts[0].shape
+    if any(tuple(t.shape) != (count, stride) for t in ts):
+        raise ValueError("batch tensors must share one (count, stride) shape")
     n_host = np.ascontiguousarray(n, dtype=np.int64)
     if n_host.shape != (count,):
         raise ValueError("n must have shape (count,)")
@@ -330,7 +397,8 @@ def rad_angular_spectrum(batch: dict, n, omega, thx, thy, d_solid_angle: float, 
         out = torch.empty(omega.numel(), dtype=torch.float64, device=omega.device)
     _check(lib.rad_angular_spectrum(ctypes.byref(b), ctypes.byref(g), int(model),
                                     lam.ctypes.data if lam is not None else None, float(d_solid_angle),
-                                    float(theta_cut), _dev(out, "out").data_ptr(), ws, nb, _stream_ptr(stream)))
+                                    float(theta_cut), _dev(out, "out").data_ptr(), ws, nb, _opt(kernel, profile),
+                                    _stream_ptr(stream)))
     return out
 
 
@@ -346,26 +414,36 @@ def _host(a, name: str) -> np.ndarray:
 
 
 def rad_eval_host(traj: dict, omega, thx, thy, model: int = CLASSICAL, hbarc_over_E: float = 0.0,
-                  out=None, stream=None):
+                  out=None, stream=None, kernel: int = 0, profile=None):
     """Host-buffer call: H2D, evaluate, D2H inside the C library."""
     hs = [_host(traj[k], k) for k in FIELDS]
     n = hs[0].shape[0]
+    if any(h.ndim != 1 or h.shape[0] != n for h in hs):
+        raise ValueError("trajectory arrays must be 1-D and of one length")
     w, x, y = _host(omega, "omega"), _host(thx, "thx"), _host(thy, "thy")
     t = _Traj(n, *[h.ctypes.data for h in hs])
     g = _Grid(w.size, x.size, y.size, w.ctypes.data, x.ctypes.data, y.ctypes.data)
     if out is None:
         out = np.empty((w.size, y.size, x.size), dtype=np.float64)
     o = _host(out, "out")
+    if o.size != w.size * x.size * y.size:
+        raise ValueError("out has the wrong number of elements")
     _check(load_library().rad_eval_host(ctypes.byref(t), ctypes.byref(g), int(model), float(hbarc_over_E),
-                                        o.ctypes.data, _stream_ptr(stream)))
+                                        o.ctypes.data, _opt(kernel, profile), _stream_ptr(stream)))
     return out
 
 
 def rad_ensemble_sum_host(batch: dict, n, omega, thx, thy, model: int = CLASSICAL, hbarc_over_E=None,
-                          accumulate: bool = False, out=None, stream=None):
+                          accumulate: bool = False, out=None, stream=None, kernel: int = 0, profile=None):
     hs = [_host(batch[k], k) for k in FIELDS]
+    if hs[0].ndim != 2:
+        raise ValueError("batch arrays must be 2-D (count, stride)")
     count, stride = hs[0].shape
+    if any(h.shape != (count, stride) for h in hs):
+        raise ValueError("batch arrays must share one (count, stride) shape")
     n_host = np.ascontiguousarray(n, dtype=np.int64)
+    if n_host.shape != (count,):
+        raise ValueError("n must have shape (count,)")
     lam = None
     if hbarc_over_E is not None:
         lam = np.ascontiguousarray(np.broadcast_to(np.asarray(hbarc_over_E, dtype=np.float64), (count,)))
@@ -377,9 +455,12 @@ def rad_ensemble_sum_host(batch: dict, n, omega, thx, thy, model: int = CLASSICA
             raise ValueError("accumulate needs an existing out")
         out = np.empty((w.size, y.size, x.size), dtype=np.float64)
     o = _host(out, "out")
+    if o.size != w.size * x.size * y.size:
+        raise ValueError("out has the wrong number of elements")
     _check(load_library().rad_ensemble_sum_host(ctypes.byref(b), ctypes.byref(g), int(model),
                                                 lam.ctypes.data if lam is not None else None,
-                                                1 if accumulate else 0, o.ctypes.data, _stream_ptr(stream)))
+                                                1 if accumulate else 0, o.ctypes.data, _opt(kernel, profile),
+                                                _stream_ptr(stream)))
     return out
 
 
@@ -395,25 +476,23 @@ def rad_launch_count() -> int:
     return int(load_library().rad_launch_count())
 
 
-def rad_set_kernel(choice: int = 0) -> None:
-    """0: choose by grid shape (default), 1: direct-phasor kernel, 2: separable-phasor kernel."""
-    _check(load_library().rad_set_kernel(int(choice)))
-
-
-def rad_plan_kernel(n_omega: int, n_thx: int, n_thy: int, model: int = CLASSICAL) -> int:
-    """1: direct-phasor kernel, 2: separable-phasor kernel, for a grid of this shape (current setting)."""
-    rc = load_library().rad_plan_kernel(n_omega, n_thx, n_thy, int(model))
+def rad_plan_kernel(n_omega: int, n_thx: int, n_thy: int, model: int = CLASSICAL, kernel: int = 0, count: int = 1,
+                    n_max: int = 1 << 20) -> int:
+    """1 direct, 2 separable, 3 fused: the kernel that takes (the largest part of) a grid of this shape for
+    `count` trajectories of at most n_max samples under the option `kernel`."""
+    rc = load_library().rad_plan_kernel(count, n_max, n_omega, n_thx, n_thy, int(model), int(kernel))
     if rc < 0:
         _check(rc)
     return rc
 
 
-def rad_plan_describe(count: int, n_max: int, n_omega: int, n_thx: int, n_thy: int, model: int = CLASSICAL) -> dict:
-    """Launch plan of a call of this shape: kernel (1 direct, 2 separable), mode (0 direct, 1 trajectory
-    slices, 2 time slices), tiles (gridDim.x), slices (gridDim.y), t_slices, chunks per trajectory."""
-    plan = (ctypes.c_int32 * 6)()
-    _check(load_library().rad_plan_describe(count, n_max, n_omega, n_thx, n_thy, int(model), plan))
-    return dict(zip(("kernel", "mode", "tiles", "slices", "t_slices", "chunks"), (int(v) for v in plan)))
+def rad_plan_describe(count: int, n_max: int, n_omega: int, n_thx: int, n_thy: int, model: int = CLASSICAL,
+                      kernel: int = 0) -> dict:
+    """Launch plan of a call of this shape (include/rad.h rad_plan_describe)."""
+    plan = (ctypes.c_int32 * 10)()
+    _check(load_library().rad_plan_describe(count, n_max, n_omega, n_thx, n_thy, int(model), int(kernel), plan))
+    keys = ("kernel", "mode", "tiles", "slices", "t_slices", "chunks", "parts", "interior_x", "interior_y", "launches")
+    return dict(zip(keys, (int(v) for v in plan)))
 
 
 def rad_formation_length(gamma: float, omega: float, hbarc_over_E: float) -> float:
@@ -422,14 +501,3 @@ def rad_formation_length(gamma: float, omega: float, hbarc_over_E: float) -> flo
     if v < 0:
         raise ValueError("rad_formation_length: need gamma >= 1, omega > 0 and hbar omega < E")
     return v
-
-
-def rad_profile_enable(on: bool = True) -> None:
-    _check(load_library().rad_profile_enable(1 if on else 0))
-
-
-def rad_profile_last():
-    """(pack_ms, main_ms, finalize_ms) of the most recent device-buffer call."""
-    ms = (ctypes.c_float * 3)()
-    _check(load_library().rad_profile_last(ms))
-    return float(ms[0]), float(ms[1]), float(ms[2])

@@ -20,13 +20,14 @@
 #include <cmath>
 #include <cstdio>
 #include <cstring>
-#include <mutex>
+#include <new>
 #include <vector>
 
 #include <cuda_runtime.h>
 
 #include "../../include/rad.h"
 #include "rad_device.cuh"
+#include "rad_plan.h"
 
 namespace rad {
 
@@ -42,8 +43,6 @@ constexpr int STAGES = 3;    // shared-memory ring depth
 constexpr int SMEM_WT = W * TPB * 16;            // per-thread omega*/2pi double-doubles, parked in smem
 constexpr int SMEM_BYTES = STAGES * CHUNK_BYTES + SMEM_WT + STAGES * 8;
 
-enum Mode : int { MODE_DIRECT = 0, MODE_PSLICE = 1, MODE_TSPLIT = 2 };
-
 struct MainParams {
     const double *packed;     // [count][cpt][CHUNK_DBL]
     const int64_t *n_dev;     // samples per trajectory (device) or nullptr -> n_single
@@ -54,10 +53,30 @@ struct MainParams {
     const double *omega, *thx, *thy;
     int n_omega, n_thx, n_thy;
     int model, mode, p_slices, t_slices, accumulate;
-    double *out;
+    double *out;              // first element of this launch's part of the cube
+    int out_nx;               // row stride of the cube (n_thx of the whole grid)
+    int64_t out_plane;        // omega stride of the cube (n_thx * n_thy of the whole grid)
     double *partial;
     int64_t t_pad;            // tiles * TPB
+    // direct kernel on the L-shaped rest of the angle plane (the separable kernel took [0, l_x0) x [0, l_y0));
+    // l_x0 < 0: the whole tensor grid.  n_thx, n_thy are the whole plane's in that case.
+    int l_x0, l_y0;
+    // angular spectrum (MODE_DIRECT only): per-(CTA, omega slot) sums over the CTA's angles instead of the cube
+    int ang, ang_groups;      // ang_groups: omega groups a CTA of the direct kernel can span
+    double cut2;              // theta_cut^2, <= 0: no mask
+    double *ang_partial;
 };
+
+// Angles a launch of the direct kernel covers, and the (i_x, i_y) of its a-th angle.
+__host__ __device__ __forceinline__ int angle_count(int n_thx, int n_thy, int l_x0, int l_y0) {
+    return l_x0 < 0 ? n_thx * n_thy : (n_thx - l_x0) * n_thy + l_x0 * (n_thy - l_y0);
+}
+__device__ __forceinline__ void angle_of(const MainParams &P, int a, int &ix, int &iy) {
+    if (P.l_x0 < 0) { ix = a % P.n_thx; iy = a / P.n_thx; return; }
+    const int rx = P.n_thx - P.l_x0, n1 = rx * P.n_thy;
+    if (a < n1) { ix = P.l_x0 + a % rx; iy = a / rx; }              // columns right of the interior, all rows
+    else { const int j = a - n1; ix = j % P.l_x0; iy = P.l_y0 + j / P.l_x0; }   // rows above it, interior columns
+}
 
 }  // namespace rad
 #include "rad_sep.cuh"
@@ -76,12 +95,20 @@ __device__ __forceinline__ dd phase_offset_dd(double gamma, double t, double dz,
     return fast_two_sum(s.hi, s.lo + at.lo);
 }
 
+__device__ __forceinline__ void pack_one(const rad_traj_batch &b, const int64_t *n_dev, int64_t n_single,
+                                         const int64_t *off_dev, int cpt, double *packed, int p, int64_t slot);
+
 __global__ void __launch_bounds__(256)
 rad_pack_kernel(rad_traj_batch b, const int64_t *n_dev, int64_t n_single, const int64_t *off_dev, int cpt,
                 double *packed) {
-    const int p = blockIdx.y;
     const int64_t slot = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
     if (slot >= (int64_t)cpt * CH) return;
+    for (int p = blockIdx.y; p < b.count; p += gridDim.y)           // gridDim.y <= 65535 trajectories at a time
+        pack_one(b, n_dev, n_single, off_dev, cpt, packed, p, slot);
+}
+
+__device__ __forceinline__ void pack_one(const rad_traj_batch &b, const int64_t *n_dev, int64_t n_single,
+                                         const int64_t *off_dev, int cpt, double *packed, int p, int64_t slot) {
     const int64_t n = n_dev ? n_dev[p] : n_single;
     const int c = (int)(slot / CH), i = (int)(slot % CH);
     const int64_t c0 = (int64_t)c * CH;
@@ -144,6 +171,76 @@ __device__ __forceinline__ double spectrum_value(const double (&acc)[NC], double
     return (0.5 * (1.0 + e * e) * S + u * u / (2.0 * gamma0 * gamma0) * J2) * INV_4PI2;
 }
 
+// ------------------------------------------------------------------------------ shared pieces of the direct kernels
+// Chunk base phase in turns, per omega, reduced to [-1/2, 1/2] (a3, the exact part):
+// psi_b = P0_b + theta^2/2 t_b - n_x x_b - n_y y_b as a double-double, times omega*/2pi (double-double, parked
+// in shared memory at wt[j * stride]).  Returns gamma[0] of the trajectory (header slot 5).
+__device__ __forceinline__ double chunk_base_phase(const double *ck, dd h, double nx, double ny,
+                                                   const double2 *wt, int stride, double (&p0)[W]) {
+    const double2 h01 = *reinterpret_cast<const double2 *>(ck);
+    const double2 h23 = *reinterpret_cast<const double2 *>(ck + 2);
+    const double2 h45 = *reinterpret_cast<const double2 *>(ck + 4);
+    dd psi = {h01.x, h01.y};                               // P0_b
+    psi = dd_add(psi, dd_mul_d(h, h23.x));                 // + theta^2/2 * t_b
+    psi = dd_add(psi, dd_neg(two_prod(nx, h23.y)));        // - n_x x_b
+    psi = dd_add(psi, dd_neg(two_prod(ny, h45.x)));        // - n_y y_b
+#pragma unroll
+    for (int j = 0; j < W; ++j) {
+        const double2 w = wt[j * stride];
+        p0[j] = dd_frac(dd_mul(dd{w.x, w.y}, psi));
+    }
+    return h45.y;
+}
+
+// One sample record against one angle and W omegas: a2 (integrand geometry, eqs. 3, 4, 6, 12), a3 (phase and
+// phasor), a4 (complex accumulation).
+template <int NC, int DEG>
+__device__ __forceinline__ void accumulate_sample(const double *rec, double nx, double ny, double hhi,
+                                                  const double (&wh)[W], const double (&p0)[W],
+                                                  double (&acc)[W][NC]) {
+    const double2 r01 = *reinterpret_cast<const double2 *>(rec);       // D0, vx
+    const double2 r23 = *reinterpret_cast<const double2 *>(rec + 2);   // vy, w ax
+    const double2 r45 = *reinterpret_cast<const double2 *>(rec + 4);   // w ay, w az
+    const double2 r67 = *reinterpret_cast<const double2 *>(rec + 6);   // dP0, dt
+    const double2 r89 = *reinterpret_cast<const double2 *>(rec + 8);   // dx, dy
+    // a2: integrand geometry, independent of omega (eqs. 3, 4, 6, 12)
+    const double D = r01.x - hhi;                  // round bracket of eqs. 3-5
+    const double ux = nx - r01.y, uy = ny - r23.x;
+    const double bx = fma(ny, uy, D);              // n_y(n_y - v_y) + D
+    const double by = fma(nx, ux, D);              // n_x(n_x - v_x) + D
+    const double q = fma(nx, ux, bx);              // eq. 6 denominator
+    const double g = inv_square(q);
+    const double s1 = fma(ny, r45.x, r45.y);       // w(az + n_y ay)
+    const double s2 = fma(nx, r23.y, r45.y);       // w(az + n_x ax)
+    const double fx = fma(s1, ux, -(bx * r23.y)) * g;      // eq. 3 (times w)
+    const double fy = fma(s2, uy, -(by * r45.x)) * g;      // eq. 4 (times w)
+    double hj = 0.0;
+    if (NC == 6) hj = fma(nx, r23.y, s1) * g;      // eq. 12 integrand (times w)
+    // eq. 7 relative to the chunk base
+    const double dpsi = fma(-ny, r89.y, fma(-nx, r89.x, fma(hhi, r67.y, r67.x)));
+#pragma unroll
+    for (int j = 0; j < W; ++j) {
+        double cs, sn;
+        phasor_turns<DEG>(fma(wh[j], dpsi, p0[j]), cs, sn);            // a3 (sn = sin/sqrt2)
+        acc[j][0] = fma(fx, cs, acc[j][0]);                              // a4
+        acc[j][1] = fma(fx, sn, acc[j][1]);
+        acc[j][2] = fma(fy, cs, acc[j][2]);
+        acc[j][3] = fma(fy, sn, acc[j][3]);
+        if (NC == 6) {
+            acc[j][4] = fma(hj, cs, acc[j][4]);
+            acc[j][5] = fma(hj, sn, acc[j][5]);
+        }
+    }
+}
+
+// theta^2 / 2 as a double-double
+__device__ __forceinline__ dd half_theta2_dd(double nx, double ny) {
+    dd xx = two_prod(nx, nx), yy = two_prod(ny, ny);
+    dd s = two_sum(xx.hi, yy.hi);
+    s = fast_two_sum(s.hi, s.lo + (xx.lo + yy.lo));
+    return {0.5 * s.hi, 0.5 * s.lo};
+}
+
 // ------------------------------------------------------------------------------ main (a0-a5)
 // NC = number of real accumulators per omega: 4 (A_x, A_y) or 6 (+ J, spin-1/2).
 template <int NC, int DEG>
@@ -156,20 +253,19 @@ rad_main_kernel(const MainParams P) {
     const int tid = threadIdx.x;
 
     // ---- this thread's grid coordinates: flattened (omega-group, angle), angle fastest
-    const int A = P.n_thx * P.n_thy;
+    const int A = angle_count(P.n_thx, P.n_thy, P.l_x0, P.l_y0);
     const int n_wg = (P.n_omega + W - 1) / W;
     const int64_t T = (int64_t)n_wg * A;
     const int64_t gid = (int64_t)blockIdx.x * TPB + tid;
     const int64_t gc = min(gid, T - 1);
     const int wg = (int)(gc / A), a = (int)(gc % A);
-    const double nx = P.thx[a % P.n_thx], ny = P.thy[a / P.n_thx];
-    dd h;                                             // theta^2 / 2, double-double
+    double nx, ny;
     {
-        dd xx = two_prod(nx, nx), yy = two_prod(ny, ny);
-        dd s = two_sum(xx.hi, yy.hi);
-        s = fast_two_sum(s.hi, s.lo + (xx.lo + yy.lo));
-        h = {0.5 * s.hi, 0.5 * s.lo};
+        int ix, iy;
+        angle_of(P, a, ix, iy);
+        nx = P.thx[ix]; ny = P.thy[iy];
     }
+    const dd h = half_theta2_dd(nx, ny);               // theta^2 / 2, double-double
     auto omega_of = [&](int j) { return P.omega[min(wg * W + j, P.n_omega - 1)]; };
 
     // ---- this CTA's slice of the (trajectory, chunk) axis
@@ -250,59 +346,13 @@ rad_main_kernel(const MainParams P) {
 
             // ---- chunk base phase in turns, per omega, reduced to [-1/2, 1/2]  (a3, exact part)
             double p0[W];
-            {
-                const double2 h01 = *reinterpret_cast<const double2 *>(ck);
-                const double2 h23 = *reinterpret_cast<const double2 *>(ck + 2);
-                const double2 h45 = *reinterpret_cast<const double2 *>(ck + 4);
-                gamma0 = h45.y;
-                dd psi = {h01.x, h01.y};                               // P0_b
-                psi = dd_add(psi, dd_mul_d(h, h23.x));                 // + theta^2/2 * t_b
-                psi = dd_add(psi, dd_neg(two_prod(nx, h23.y)));        // - n_x x_b
-                psi = dd_add(psi, dd_neg(two_prod(ny, h45.x)));        // - n_y y_b
-#pragma unroll
-                for (int j = 0; j < W; ++j) {
-                    const double2 wt = wt_sm[j * TPB + tid];
-                    p0[j] = dd_frac(dd_mul(dd{wt.x, wt.y}, psi));
-                }
-            }
+            gamma0 = chunk_base_phase(ck, h, nx, ny, wt_sm + tid, TPB, p0);
 
             // ---- samples of the chunk
             const double *rec = ck + HDR;
 #pragma unroll 1
             for (int k = 0; k < CH; ++k, rec += REC) {
-                const double2 r01 = *reinterpret_cast<const double2 *>(rec);       // D0, vx
-                const double2 r23 = *reinterpret_cast<const double2 *>(rec + 2);   // vy, w ax
-                const double2 r45 = *reinterpret_cast<const double2 *>(rec + 4);   // w ay, w az
-                const double2 r67 = *reinterpret_cast<const double2 *>(rec + 6);   // dP0, dt
-                const double2 r89 = *reinterpret_cast<const double2 *>(rec + 8);   // dx, dy
-                // a2: integrand geometry, independent of omega (eqs. 3, 4, 6, 12)
-                const double D = r01.x - h.hi;                 // round bracket of eqs. 3-5
-                const double ux = nx - r01.y, uy = ny - r23.x;
-                const double bx = fma(ny, uy, D);              // n_y(n_y - v_y) + D
-                const double by = fma(nx, ux, D);              // n_x(n_x - v_x) + D
-                const double q = fma(nx, ux, bx);              // eq. 6 denominator
-                const double g = inv_square(q);
-                const double s1 = fma(ny, r45.x, r45.y);       // w(az + n_y ay)
-                const double s2 = fma(nx, r23.y, r45.y);       // w(az + n_x ax)
-                const double fx = fma(s1, ux, -(bx * r23.y)) * g;      // eq. 3 (times w)
-                const double fy = fma(s2, uy, -(by * r45.x)) * g;      // eq. 4 (times w)
-                double hj = 0.0;
-                if (NC == 6) hj = fma(nx, r23.y, s1) * g;      // eq. 12 integrand (times w)
-                // eq. 7 relative to the chunk base
-                const double dpsi = fma(-ny, r89.y, fma(-nx, r89.x, fma(h.hi, r67.y, r67.x)));
-#pragma unroll
-                for (int j = 0; j < W; ++j) {
-                    double cs, sn;
-                    phasor_turns<DEG>(fma(wh[j], dpsi, p0[j]), cs, sn);            // a3 (sn = sin/sqrt2)
-                    acc[j][0] = fma(fx, cs, acc[j][0]);                              // a4
-                    acc[j][1] = fma(fx, sn, acc[j][1]);
-                    acc[j][2] = fma(fy, cs, acc[j][2]);
-                    acc[j][3] = fma(fy, sn, acc[j][3]);
-                    if (NC == 6) {
-                        acc[j][4] = fma(hj, cs, acc[j][4]);
-                        acc[j][5] = fma(hj, sn, acc[j][5]);
-                    }
-                }
+                accumulate_sample<NC, DEG>(rec, nx, ny, h.hi, wh, p0, acc);
             }
             __syncthreads();                          // every thread is done with stage s
             if (tid == 0) produce();
@@ -326,15 +376,59 @@ rad_main_kernel(const MainParams P) {
         double *dst = P.partial + (int64_t)slice * W * P.t_pad + gid;
 #pragma unroll
         for (int j = 0; j < W; ++j) dst[(int64_t)j * P.t_pad] = S_sum[j];
+    } else if (P.mode == MODE_DIRECT && P.ang) {
+        // ---- angular spectrum: sum of this CTA's angles per omega, in thread order (N1)
+        __syncthreads();                              // the ring is free: every chunk has been consumed
+        double *red = ring;                           // [TPB][W]
+        const bool inside = gid < T && (P.cut2 <= 0.0 || fma(nx, nx, ny * ny) <= P.cut2);
+#pragma unroll
+        for (int j = 0; j < W; ++j) red[tid * W + j] = inside ? S_sum[j] : 0.0;
+        __syncthreads();
+        const int64_t g0 = (int64_t)blockIdx.x * TPB;
+        const int wg_first = (int)(g0 / A);
+        for (int slot = tid; slot < P.ang_groups * W; slot += TPB) {
+            const int g = slot / W, j = slot % W;
+            const int64_t lo = max(g0, (int64_t)(wg_first + g) * A), hi = min(g0 + TPB, (int64_t)(wg_first + g + 1) * A);
+            double sum = 0.0;
+            for (int64_t t = lo; t < hi; ++t) sum += red[(int)(t - g0) * W + j];
+            P.ang_partial[((int64_t)blockIdx.x * P.ang_groups + g) * W + j] = sum;
+        }
     } else if (P.mode == MODE_DIRECT && gid < T) {
+        int ix, iy;                                   // (recomputed: not kept in registers across the time loop)
+        angle_of(P, a, ix, iy);
 #pragma unroll
         for (int j = 0; j < W; ++j) {
             const int iw = wg * W + j;
             if (iw < P.n_omega) {
-                double *o = P.out + (int64_t)iw * A + a;
+                double *o = P.out + iw * P.out_plane + (int64_t)iy * P.out_nx + ix;
                 *o = P.accumulate ? *o + S_sum[j] : S_sum[j];
             }
         }
+    }
+}
+
+// angular spectrum, second pass for the direct kernel: spec[i_w] (+)= d_solid * sum over the tiles that hold
+// omega group i_w / W, in ascending tile order.  One CTA per omega: 256 threads sum contiguous blocks of tiles,
+// thread 0 adds the 256 block sums in order (fixed order: deterministic).
+__global__ void __launch_bounds__(256)
+rad_ang_final_direct_kernel(const double *partial, int A, int groups, int n_omega, double d_solid, int accumulate,
+                            double *spec) {
+    __shared__ double red[256];
+    const int iw = blockIdx.x, wg = iw / W, j = iw % W;
+    const int64_t t_lo = (int64_t)wg * A / TPB, t_hi = ((int64_t)(wg + 1) * A - 1) / TPB + 1;    // tiles [t_lo, t_hi)
+    const int64_t per = (t_hi - t_lo + 255) / 256;
+    double s = 0.0;
+    for (int64_t t = t_lo + threadIdx.x * per; t < min(t_hi, t_lo + (threadIdx.x + 1) * per); ++t) {
+        const int g = wg - (int)(t * TPB / A);
+        s += partial[(t * groups + g) * W + j];
+    }
+    red[threadIdx.x] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double tot = 0.0;
+        for (int k = 0; k < 256; ++k) tot += red[k];
+        tot *= d_solid;
+        spec[iw] = accumulate ? spec[iw] + tot : tot;
     }
 }
 
@@ -342,13 +436,15 @@ rad_main_kernel(const MainParams P) {
 template <int NC>
 __global__ void __launch_bounds__(TPB)
 rad_finalize_kernel(const MainParams P) {
-    const int A = P.n_thx * P.n_thy;
+    const int A = angle_count(P.n_thx, P.n_thy, P.l_x0, P.l_y0);
     const int n_wg = (P.n_omega + W - 1) / W;
     const int64_t T = (int64_t)n_wg * A;
     const int64_t gid = (int64_t)blockIdx.x * TPB + threadIdx.x;
     if (gid >= T) return;
     const int wg = (int)(gid / A), a = (int)(gid % A);
-    const double nx = P.thx[a % P.n_thx], ny = P.thy[a / P.n_thx];
+    int ix, iy;
+    angle_of(P, a, ix, iy);
+    const double nx = P.thx[ix], ny = P.thy[iy];
     {                                                 // gridDim.y = W: one omega of the register tile per CTA row
         const int j = blockIdx.y;
         const int iw = wg * W + j;
@@ -373,10 +469,14 @@ rad_finalize_kernel(const MainParams P) {
                 total += spectrum_value<NC>(acc, nx, ny, P.model, om * lam, gamma0);
             }
         }
-        double *o = P.out + (int64_t)iw * A + a;
+        double *o = P.out + iw * P.out_plane + (int64_t)iy * P.out_nx + ix;
         *o = P.accumulate ? *o + total : total;
     }
 }
+
+}  // namespace rad
+#include "rad_fused.cuh"
+namespace rad {
 
 // ------------------------------------------------------------------------------ angular sum
 // one CTA per omega; fixed-order tree reduction in shared memory (deterministic)
@@ -398,6 +498,14 @@ rad_angular_sum_kernel(const double *cube, const double *thx, const double *thy,
         __syncthreads();
     }
     if (threadIdx.x == 0) spec[blockIdx.x] = red[0] * d_solid;
+}
+
+// ------------------------------------------------------------------------------ number spectrum
+// dN/dw = (dI/dw) / (hbar w), PAPER.md:50-56 (eq. 8 is stated for the number spectrum)
+__global__ void __launch_bounds__(256)
+rad_number_spectrum_kernel(const double *spec, const double *omega, int n, double hbar_c, double *number) {
+    const int i = blockIdx.x * blockDim.x + threadIdx.x;
+    if (i < n) number[i] = spec[i] / (hbar_c * omega[i]);
 }
 
 // ------------------------------------------------------------------------------ ordered cube sum
@@ -433,25 +541,6 @@ rad_fma_peak_kernel(double *sink, int iters, double a, double b) {
 static std::atomic<int64_t> g_launches{0};
 static thread_local char g_err[256] = "no CUDA error recorded";
 
-// Optional per-kernel timing of the last call (bench.py's roofline needs the main kernel's own
-// duration): events recorded on the caller's stream around pack / main / finalize.
-static std::atomic<int> g_prof{0};
-static cudaEvent_t g_ev[4];
-static bool g_ev_ready = false, g_ev_have_finalize = false;
-static std::mutex g_ev_mu;
-
-static void prof_mark(int i, cudaStream_t st) {
-    if (!g_prof.load()) return;
-    std::lock_guard<std::mutex> lk(g_ev_mu);
-    if (!g_ev_ready) {
-        for (auto &e : g_ev) cudaEventCreate(&e);
-        g_ev_ready = true;
-    }
-    cudaEventRecord(g_ev[i], st);
-    if (i == 2) g_ev_have_finalize = false;
-    if (i == 3) g_ev_have_finalize = true;
-}
-
 static int cuda_fail(cudaError_t e, const char *what) {
     snprintf(g_err, sizeof g_err, "%s: %s", what, cudaGetErrorString(e));
     return RAD_ECUDA;
@@ -462,17 +551,77 @@ static int cuda_fail(cudaError_t e, const char *what) {
         if (e_ != cudaSuccess) return cuda_fail(e_, #call);   \
     } while (0)
 
+// ---- per-device facts and one-time setup, keyed by the current device (one process may drive several GPUs)
+constexpr int MAX_DEV = 64;
+struct DeviceState {
+    std::atomic<int> sms{0};
+    std::atomic<int> fused_resident[2];               // co-resident CTAs of rad_fused_kernel<4>, <6>; 0 = not asked yet
+    std::atomic<unsigned> attr_done{0};               // bit per kernel whose dynamic shared-memory limit is set
+    std::atomic<int> pool_done{0};
+};
+static DeviceState g_dev[MAX_DEV];
+
+static int current_device() {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return -1; }
+    return dev >= 0 && dev < MAX_DEV ? dev : -1;
+}
+
 static int sm_count() {
-    static int n = 0;
+    const int dev = current_device();
+    if (dev < 0) return 0;
+    int n = g_dev[dev].sms.load();
     if (n == 0) {
-        int dev = 0;
-        if (cudaGetDevice(&dev) != cudaSuccess) return 0;
-        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) n = 0;
+        if (cudaDeviceGetAttribute(&n, cudaDevAttrMultiProcessorCount, dev) != cudaSuccess) { cudaGetLastError(); n = 0; }
+        g_dev[dev].sms.store(n);
     }
     return n;
 }
 
-static size_t align_up(size_t v, size_t a) { return (v + a - 1) / a * a; }
+template <typename K>
+static cudaError_t ensure_smem(K kernel, int bit, int bytes) {
+    const int dev = current_device();
+    if (dev < 0) return cudaErrorNoDevice;
+    if (g_dev[dev].attr_done.load() & (1u << bit)) return cudaSuccess;
+    const cudaError_t e = cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, bytes);
+    if (e == cudaSuccess) g_dev[dev].attr_done.fetch_or(1u << bit);
+    return e;
+}
+
+// CTAs of the fused kernel the current device holds at once (0: no device / error -> the planner assumes 4 per SM)
+template <int NC>
+static int fused_resident() {
+    const int dev = current_device();
+    if (dev < 0) return 0;
+    std::atomic<int> &slot = g_dev[dev].fused_resident[NC == 6];
+    int v = slot.load();
+    if (v == 0) {
+        int per_sm = 0;
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rad_fused_kernel<NC, RAD_DEG>, FUSED_TPB, FUSED_SMEM)
+            != cudaSuccess) { cudaGetLastError(); per_sm = 0; }
+        v = per_sm * sm_count();
+        slot.store(v > 0 ? v : -1);
+    }
+    return v > 0 ? v : 0;
+}
+static int fused_resident_for(int nc) {
+    const int v = nc == 6 ? fused_resident<6>() : fused_resident<4>();
+    return v > 0 ? v : 4 * 148;                       // no device: plan as for a B200
+}
+
+// ---- per-call timing (rad_options.profile)
+}  // namespace rad
+struct rad_profile {
+    cudaEvent_t ev[4];
+    bool have_reduce;
+};
+namespace rad {
+static void prof_mark(rad_profile *pr, int i, cudaStream_t st) {
+    if (!pr) return;
+    cudaEventRecord(pr->ev[i], st);
+    if (i == 0) pr->have_reduce = false;
+    if (i == 3) pr->have_reduce = true;
+}
 
 // Scratch taken from the stream-ordered pool goes back in stream order on every exit path.
 struct PoolScratch {
@@ -480,120 +629,36 @@ struct PoolScratch {
     cudaStream_t st = nullptr;
     ~PoolScratch() { if (p) cudaFreeAsync(p, st); }
 };
-
-// The launch plan is a pure function of the shapes (and the SM count, 148 assumed when no
-// device is visible so that rad_workspace_bytes works on a CPU-only box).
-struct Plan {
-    int kernel;               // 0: rad_main_kernel (one phasor per eval), 1: rad_sep_kernel (separable phasor)
-    int cpt, tiles, p_slices, t_slices, mode;
-    int64_t t_pad;
-    size_t off_packed, off_n, off_lam, off_start, off_partial, total;
-};
-
-static std::atomic<int> g_kernel_choice{0};          // rad_set_kernel: 0 auto, 1 direct, 2 separable
-
-// The separable kernel works on tiles of 16 omega x 16 n_x x (16 or 8) n_y points: use it when padding
-// the grid to whole tiles wastes less work than the kernel saves (it needs about half the FP64
-// instructions per eval of the direct kernel).
-static int choose_kernel(int n_omega, int n_thx, int n_thy, int nc) {
-    const int choice = g_kernel_choice.load();
-    if (choice == 1) return 0;
-    if (choice == 2) return 1;
-    const int ty = nc == 6 ? 8 : 16;
-    const double padded = (double)((n_omega + 15) / 16 * 16) * ((n_thx + 15) / 16 * 16) * ((n_thy + ty - 1) / ty * ty);
-    // measured speed-up of the separable kernel on full tiles: 1.8x (4 accumulators per point), 1.4x (6)
-    const double break_even = nc == 6 ? 0.75 : 0.6;
-    return (double)n_omega * n_thx * n_thy >= break_even * padded ? 1 : 0;
-}
-
-static Plan make_plan(int count, int64_t n_max, int n_omega, int n_thx, int n_thy, int nc, int kernel) {
-    Plan pl{};
-    pl.kernel = kernel;
-    int sms = sm_count();
-    if (sms <= 0) sms = 148;
-    pl.cpt = (int)((n_max + CH - 1) / CH);
-    pl.p_slices = 1; pl.t_slices = 1; pl.mode = MODE_DIRECT;
-    size_t per_thread_p, per_thread_t;                // partial doubles per thread and slice
-    if (kernel == 0) {
-        const int64_t T = (int64_t)((n_omega + W - 1) / W) * n_thx * n_thy;
-        pl.tiles = (int)((T + TPB - 1) / TPB);
-        pl.t_pad = (int64_t)pl.tiles * TPB;
-        per_thread_p = W; per_thread_t = (size_t)nc * W;
-        // two CTAs per SM: the fewest slices k (>= 2 waves of work) whose tiles*k CTAs fill whole
-        // waves of 2 * sms to >= 98.5 %
-        const int slots = 2 * sms;
-        if (pl.tiles < 8 * sms) {
-            const int64_t kmax = std::max<int64_t>(1, (int64_t)count * std::max(1, pl.cpt));
-            int best_k = 1;
-            double best = 0.0;
-            for (int64_t k = 1; k <= std::min<int64_t>(kmax, 8 * sms); ++k) {
-                const int64_t ctas = (int64_t)pl.tiles * k;
-                double eff = (double)ctas / (double)((ctas + slots - 1) / slots * slots);
-                if (ctas < 2 * slots && k < kmax) eff *= 0.5;        // too few CTAs to balance: keep looking
-                if (eff > best + 1e-9) { best = eff; best_k = (int)k; }
-                if (eff >= 0.985) break;
-            }
-            if (best_k > 1) {
-                if (count >= best_k) { pl.mode = MODE_PSLICE; pl.p_slices = best_k; }
-                else {
-                    int ts = std::min((best_k + count - 1) / count, std::max(1, pl.cpt));
-                    if (ts > 1) { pl.mode = MODE_TSPLIT; pl.t_slices = ts; pl.p_slices = count; }
-                    else if (count > 1) { pl.mode = MODE_PSLICE; pl.p_slices = count; }
-                }
-            }
+static cudaError_t pool_alloc(void **p, size_t bytes, cudaStream_t st) {
+    // keep freed scratch cached in the device's stream-ordered pool: with the default release threshold (0)
+    // every synchronisation hands it back to the driver and the next call pays a fresh allocation
+    // (measured: 3x slower steps on cfg 2)
+    const int dev = current_device();
+    if (dev >= 0 && !g_dev[dev].pool_done.exchange(1)) {
+        cudaMemPool_t pool;
+        if (cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
+            uint64_t keep = UINT64_MAX;
+            cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
         }
-    } else {
-        const int wy = nc == 6 ? 2 : 4, ev = 4 * wy;
-        pl.tiles = ((n_omega + 15) / 16) * ((n_thx + 15) / 16) * ((n_thy + 4 * wy - 1) / (4 * wy));
-        pl.t_pad = (int64_t)pl.tiles * SEP_CONS;
-        per_thread_p = ev; per_thread_t = (size_t)nc * ev;
-        // one CTA per SM: the fewest slices k whose tiles*k CTAs fill whole waves to >= 98.5 %
-        if (pl.tiles < 8 * sms) {
-            const int64_t kmax = std::max<int64_t>(1, (int64_t)count * std::max(1, pl.cpt / 2));
-            int best_k = 1;
-            double best = 0.0;
-            for (int64_t k = 1; k <= std::min<int64_t>(kmax, 4 * sms); ++k) {
-                const int64_t ctas = (int64_t)pl.tiles * k;
-                const double eff = (double)ctas / (double)((ctas + sms - 1) / sms * sms);
-                if (eff > best + 1e-9) { best = eff; best_k = (int)k; }
-                if (eff >= 0.985) break;
-            }
-            if (best_k > 1) {
-                if (count >= best_k) { pl.mode = MODE_PSLICE; pl.p_slices = best_k; }
-                else {
-                    int ts = std::min((best_k + count - 1) / count, std::max(1, pl.cpt / 2));
-                    if (ts > 1) { pl.mode = MODE_TSPLIT; pl.t_slices = ts; pl.p_slices = count; }
-                    else if (count > 1) { pl.mode = MODE_PSLICE; pl.p_slices = count; }
-                }
-            }
-        }
+        cudaGetLastError();
     }
-    size_t off = 0;
-    pl.off_packed = off; off += align_up((size_t)count * pl.cpt * CHUNK_BYTES, 256);
-    pl.off_n = off;      off += align_up((size_t)count * sizeof(int64_t), 256);
-    pl.off_lam = off;    off += align_up((size_t)count * sizeof(double), 256);
-    pl.off_start = off;  off += align_up((size_t)count * sizeof(int64_t), 256);
-    pl.off_partial = off;
-    if (pl.mode == MODE_PSLICE) off += align_up((size_t)pl.p_slices * per_thread_p * pl.t_pad * 8, 256);
-    if (pl.mode == MODE_TSPLIT) off += align_up((size_t)count * pl.t_slices * per_thread_t * pl.t_pad * 8, 256);
-    pl.total = off;
-    return pl;
+    return cudaMallocAsync(p, bytes, st);
 }
 
 static bool grid_ok(const rad_grid *g) {
     return g && g->n_omega > 0 && g->n_thx > 0 && g->n_thy > 0 && g->omega && g->thx && g->thy;
 }
 static bool aligned8(const void *p) { return (reinterpret_cast<uintptr_t>(p) & 7) == 0; }
+static int kernel_option(const rad_options *opt) { return opt ? opt->kernel : 0; }
+
+static CallPlan plan_for(int count, int64_t n_max, int n_omega, int n_thx, int n_thy, int nc, int kernel, bool angular) {
+    return plan_call(count, n_max, n_omega, n_thx, n_thy, nc, kernel, angular, sm_count(), fused_resident_for(nc));
+}
 
 template <int NC, int DEG>
 static cudaError_t launch_main(const MainParams &mp, dim3 grid, cudaStream_t st) {
-    static std::once_flag once;
-    static cudaError_t attr_err = cudaSuccess;
-    std::call_once(once, [] {
-        attr_err = cudaFuncSetAttribute(rad_main_kernel<NC, DEG>,
-                                        cudaFuncAttributeMaxDynamicSharedMemorySize, SMEM_BYTES);
-    });
-    if (attr_err != cudaSuccess) return attr_err;
+    const cudaError_t a = ensure_smem(rad_main_kernel<NC, DEG>, NC == 6 ? 1 : 0, SMEM_BYTES);
+    if (a != cudaSuccess) return a;
     rad_main_kernel<NC, DEG><<<grid, TPB, SMEM_BYTES, st>>>(mp);
     ++g_launches;
     return cudaGetLastError();
@@ -601,31 +666,40 @@ static cudaError_t launch_main(const MainParams &mp, dim3 grid, cudaStream_t st)
 
 template <int NC, int WY>
 static cudaError_t launch_sep(const MainParams &mp, dim3 grid, cudaStream_t st) {
-    static std::once_flag once;
-    static cudaError_t attr_err = cudaSuccess;
-    std::call_once(once, [] {
-        attr_err = cudaFuncSetAttribute(rad_sep_kernel<NC, WY>, cudaFuncAttributeMaxDynamicSharedMemorySize,
-                                        SepShape<NC, WY>::SMEM);
-    });
-    if (attr_err != cudaSuccess) return attr_err;
+    const cudaError_t a = ensure_smem(rad_sep_kernel<NC, WY>, NC == 6 ? 3 : 2, SepShape<NC, WY>::SMEM);
+    if (a != cudaSuccess) return a;
     rad_sep_kernel<NC, WY><<<grid, SepRegs<NC>::THREADS, SepShape<NC, WY>::SMEM, st>>>(mp);
     ++g_launches;
     return cudaGetLastError();
 }
 
-// Everything: pack, main, finalize.  All device pointers; n_host / lam_host are host arrays.
+template <int NC>
+static cudaError_t launch_fused(FusedParams &fp, cudaStream_t st) {
+    void *args[] = {&fp};
+    const cudaError_t e = cudaLaunchCooperativeKernel(reinterpret_cast<const void *>(rad_fused_kernel<NC, RAD_DEG>),
+                                                      dim3(fp.tiles, fp.slices), dim3(FUSED_TPB), args, FUSED_SMEM, st);
+    ++g_launches;
+    return e;
+}
+
+// Everything: pack, main, ordered reduction.  All device pointers; n_host / lam_host are host arrays.
 // off_host (optional): first sample of each trajectory inside the arrays (sections of one long trajectory);
-// NULL: row p starts at p * stride.
+// NULL: row p starts at p * stride.  ang != nullptr: the angular spectrum instead of the cube (the caller has
+// checked that the plan is one part in MODE_DIRECT).
+struct AngularOut { double d_solid, cut2; double *spectrum; };
+
 static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const int64_t *off_host, const rad_grid *g,
-                     int model, const double *lam_host, int accumulate, double *out,
-                     void *workspace, size_t workspace_bytes, cudaStream_t st) {
-    if (!b || b->count < 1 || !n_host || !grid_ok(g) || !out) return RAD_EINVAL;
+                     int model, const double *lam_host, int accumulate, double *out, const AngularOut *ang,
+                     void *workspace, size_t workspace_bytes, const rad_options *opt, cudaStream_t st) {
+    if (!b || b->count < 1 || !n_host || !grid_ok(g) || (!out && !ang)) return RAD_EINVAL;
     if (model < RAD_CLASSICAL || model > RAD_SPIN_HALF) return RAD_EINVAL;
     if (model != RAD_CLASSICAL && !lam_host) return RAD_EINVAL;
+    const int kopt = kernel_option(opt);
+    if (kopt < RAD_KERNEL_AUTO || kopt > RAD_KERNEL_FUSED || (opt && opt->reserved != 0)) return RAD_EINVAL;
     const double *arrs[11] = {b->t, b->dz, b->x, b->y, b->vx, b->vy, b->dvz, b->ax, b->ay, b->az, b->gamma};
     for (const double *p : arrs)
         if (!p || !aligned8(p)) return RAD_EINVAL;
-    if (!aligned8(out) || !aligned8(g->omega) || !aligned8(g->thx) || !aligned8(g->thy)) return RAD_EINVAL;
+    if ((out && !aligned8(out)) || !aligned8(g->omega) || !aligned8(g->thx) || !aligned8(g->thy)) return RAD_EINVAL;
     int64_t n_max = 0;
     for (int p = 0; p < b->count; ++p) {
         if (n_host[p] < 2 || n_host[p] > b->stride) return RAD_EINVAL;
@@ -634,95 +708,136 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const int64
         if (model != RAD_CLASSICAL && !(lam_host[p] >= 0.0)) return RAD_EDOMAIN;
     }
     const int nc = model == RAD_SPIN_HALF ? 6 : 4;
-    const Plan pl = make_plan(b->count, n_max, g->n_omega, g->n_thx, g->n_thy, nc,
-                              choose_kernel(g->n_omega, g->n_thx, g->n_thy, nc));
+    const CallPlan cp = plan_for(b->count, n_max, g->n_omega, g->n_thx, g->n_thy, nc, kopt, ang != nullptr);
+    if (kopt == RAD_KERNEL_FUSED && (!cp.fused || off_host)) return RAD_EINVAL;
+    const bool fused = cp.fused && !off_host;
+    if (ang && !(cp.nparts == 1 && cp.part[0].plan.mode == MODE_DIRECT)) return RAD_EINVAL;
     if (workspace && (reinterpret_cast<uintptr_t>(workspace) & 255)) return RAD_EINVAL;
-    if (workspace && workspace_bytes < pl.total) return RAD_ENOSPACE;
+    if (workspace && workspace_bytes < cp.total) return RAD_ENOSPACE;
     PoolScratch pool;
     char *ws = static_cast<char *>(workspace);
     if (!ws) {
-        // keep freed scratch cached in the device's stream-ordered pool: with the default release
-        // threshold (0) every synchronisation hands it back to the driver and the next call pays a
-        // fresh allocation (measured: 3x slower steps on cfg 2)
-        static std::once_flag pool_once;
-        std::call_once(pool_once, [] {
-            int dev = 0;
-            cudaMemPool_t pool;
-            if (cudaGetDevice(&dev) == cudaSuccess && cudaDeviceGetDefaultMemPool(&pool, dev) == cudaSuccess) {
-                uint64_t keep = UINT64_MAX;
-                cudaMemPoolSetAttribute(pool, cudaMemPoolAttrReleaseThreshold, &keep);
-            }
-            cudaGetLastError();
-        });
         void *pnew = nullptr;
-        CK(cudaMallocAsync(&pnew, pl.total, st));
+        CK(pool_alloc(&pnew, cp.total, st));
         ws = static_cast<char *>(pnew);
         pool.p = pnew; pool.st = st;
     }
-    double *packed = reinterpret_cast<double *>(ws + pl.off_packed);
+    rad_profile *prof = opt ? opt->profile : nullptr;
+
+    if (fused) {              // ---- one cooperative launch does rows a0-a6 (rad_fused.cuh)
+        FusedParams fp{};
+        fp.tr = rad_traj{n_host[0], b->t, b->dz, b->x, b->y, b->vx, b->vy, b->dvz, b->ax, b->ay, b->az, b->gamma};
+        fp.lam = model == RAD_CLASSICAL ? 0.0 : lam_host[0];
+        fp.omega = g->omega; fp.thx = g->thx; fp.thy = g->thy;
+        fp.n_omega = g->n_omega; fp.n_thx = g->n_thx; fp.n_thy = g->n_thy;
+        fp.model = model; fp.accumulate = accumulate ? 1 : 0;
+        fp.tiles = cp.fused_tiles; fp.slices = cp.fused_slices;
+        fp.partial = reinterpret_cast<double *>(ws + cp.part[0].off_partial);
+        fp.out = out;
+        prof_mark(prof, 0, st);
+        prof_mark(prof, 1, st);
+        const cudaError_t e = nc == 6 ? launch_fused<6>(fp, st) : launch_fused<4>(fp, st);
+        if (e != cudaSuccess) return cuda_fail(e, "rad_fused_kernel");
+        prof_mark(prof, 2, st);
+        return RAD_OK;
+    }
+
+    double *packed = reinterpret_cast<double *>(ws + cp.off_packed);
     int64_t *n_dev = nullptr;
     double *lam_dev = nullptr;
     int64_t *off_dev = nullptr;
     if (off_host) {
-        off_dev = reinterpret_cast<int64_t *>(ws + pl.off_start);
+        off_dev = reinterpret_cast<int64_t *>(ws + cp.off_start);
         CK(cudaMemcpyAsync(off_dev, off_host, (size_t)b->count * sizeof(int64_t), cudaMemcpyHostToDevice, st));
     }
     if (b->count > 1) {
-        n_dev = reinterpret_cast<int64_t *>(ws + pl.off_n);
+        n_dev = reinterpret_cast<int64_t *>(ws + cp.off_n);
         CK(cudaMemcpyAsync(n_dev, n_host, (size_t)b->count * sizeof(int64_t), cudaMemcpyHostToDevice, st));
         if (model != RAD_CLASSICAL) {
-            lam_dev = reinterpret_cast<double *>(ws + pl.off_lam);
+            lam_dev = reinterpret_cast<double *>(ws + cp.off_lam);
             CK(cudaMemcpyAsync(lam_dev, lam_host, (size_t)b->count * sizeof(double), cudaMemcpyHostToDevice, st));
         }
     }
-    prof_mark(0, st);
+    prof_mark(prof, 0, st);
     {   // a0/a1: pack
-        dim3 grid((unsigned)(((int64_t)pl.cpt * CH + 255) / 256), (unsigned)b->count);
-        rad_pack_kernel<<<grid, 256, 0, st>>>(*b, n_dev, n_host[0], off_dev, pl.cpt, packed);
+        dim3 grid((unsigned)(((int64_t)cp.cpt * CH + 255) / 256), (unsigned)std::min(b->count, 65535));
+        rad_pack_kernel<<<grid, 256, 0, st>>>(*b, n_dev, n_host[0], off_dev, cp.cpt, packed);
         ++g_launches;
         CK(cudaGetLastError());
     }
-    prof_mark(1, st);
-    MainParams mp{};
-    mp.packed = packed; mp.n_dev = n_dev; mp.lam_dev = lam_dev;
-    mp.n_single = n_host[0];
-    mp.lam_single = model == RAD_CLASSICAL ? 0.0 : lam_host[0];
-    mp.count = b->count; mp.cpt = pl.cpt;
-    mp.omega = g->omega; mp.thx = g->thx; mp.thy = g->thy;
-    mp.n_omega = g->n_omega; mp.n_thx = g->n_thx; mp.n_thy = g->n_thy;
-    mp.model = model; mp.mode = pl.mode; mp.p_slices = pl.p_slices; mp.t_slices = pl.t_slices;
-    mp.accumulate = accumulate ? 1 : 0;
-    mp.out = out; mp.partial = reinterpret_cast<double *>(ws + pl.off_partial);
-    mp.t_pad = pl.t_pad;
-    const int slices = pl.mode == MODE_TSPLIT ? b->count * pl.t_slices : pl.p_slices;
-    dim3 grid((unsigned)pl.tiles, (unsigned)slices);
-    cudaError_t e;
-    if (pl.kernel == 1) e = nc == 6 ? launch_sep<6, 2>(mp, grid, st) : launch_sep<4, 4>(mp, grid, st);
-    else e = nc == 6 ? launch_main<6, RAD_DEG>(mp, grid, st) : launch_main<4, RAD_DEG>(mp, grid, st);
-    if (e != cudaSuccess) return cuda_fail(e, pl.kernel == 1 ? "rad_sep_kernel" : "rad_main_kernel");
-    prof_mark(2, st);
-    if (pl.mode != MODE_DIRECT) {
-        if (pl.kernel == 1) {
-            if (nc == 6) rad_sep_finalize_kernel<6, 2><<<dim3(pl.tiles, 8), SEP_CONS, 0, st>>>(mp);
-            else rad_sep_finalize_kernel<4, 4><<<dim3(pl.tiles, 16), SEP_CONS, 0, st>>>(mp);
-        } else {
-            if (nc == 6) rad_finalize_kernel<6><<<dim3(pl.tiles, W), TPB, 0, st>>>(mp);
-            else rad_finalize_kernel<4><<<dim3(pl.tiles, W), TPB, 0, st>>>(mp);
+    prof_mark(prof, 1, st);
+    MainParams mps[2];
+    for (int i = 0; i < cp.nparts; ++i) {             // main kernels of all parts first, then their reductions
+        const Part &pt = cp.part[i];
+        const Plan &pl = pt.plan;
+        MainParams &mp = mps[i];
+        mp = MainParams{};
+        mp.packed = packed; mp.n_dev = n_dev; mp.lam_dev = lam_dev;
+        mp.n_single = n_host[0];
+        mp.lam_single = model == RAD_CLASSICAL ? 0.0 : lam_host[0];
+        mp.count = b->count; mp.cpt = cp.cpt;
+        mp.omega = g->omega; mp.thx = g->thx; mp.thy = g->thy;
+        mp.n_omega = g->n_omega; mp.n_thx = pt.n_thx; mp.n_thy = pt.n_thy;
+        mp.model = model; mp.mode = pl.mode; mp.p_slices = pl.p_slices; mp.t_slices = pl.t_slices;
+        mp.accumulate = accumulate ? 1 : 0;
+        mp.out = out; mp.out_nx = g->n_thx; mp.out_plane = (int64_t)g->n_thx * g->n_thy;
+        mp.partial = reinterpret_cast<double *>(ws + pt.off_partial);
+        mp.t_pad = pl.t_pad;
+        mp.l_x0 = pt.l_x0; mp.l_y0 = pt.l_y0;
+        if (ang) {
+            mp.ang = 1; mp.cut2 = ang->cut2;
+            mp.ang_groups = std::min((g->n_omega + W - 1) / W, (TPB + pt.angles - 1) / pt.angles + 1);
+            mp.ang_partial = reinterpret_cast<double *>(ws + cp.off_ang);
         }
-        ++g_launches;
-        CK(cudaGetLastError());
-        prof_mark(3, st);
+        dim3 grid((unsigned)pl.tiles, (unsigned)pl.slices());
+        cudaError_t e;
+        if (pt.kernel == K_SEP) e = nc == 6 ? launch_sep<6, 2>(mp, grid, st) : launch_sep<4, 4>(mp, grid, st);
+        else e = nc == 6 ? launch_main<6, RAD_DEG>(mp, grid, st) : launch_main<4, RAD_DEG>(mp, grid, st);
+        if (e != cudaSuccess) return cuda_fail(e, pt.kernel == K_SEP ? "rad_sep_kernel" : "rad_main_kernel");
     }
+    prof_mark(prof, 2, st);
+    bool reduced = false;
+    for (int i = 0; i < cp.nparts; ++i) {
+        const Part &pt = cp.part[i];
+        const Plan &pl = pt.plan;
+        const MainParams &mp = mps[i];
+        if (ang) {
+            if (pt.kernel == K_SEP) {
+                const int wy = nc == 6 ? 2 : 4;
+                const int angle_tiles = ((pt.n_thx + 15) / 16) * ((pt.n_thy + 4 * wy - 1) / (4 * wy));
+                rad_ang_final_sep_kernel<<<g->n_omega, 256, 0, st>>>(mp.ang_partial, angle_tiles, g->n_omega,
+                                                                     ang->d_solid, 0, ang->spectrum);
+            } else {
+                rad_ang_final_direct_kernel<<<g->n_omega, 256, 0, st>>>(mp.ang_partial, pt.angles, mp.ang_groups,
+                                                                        g->n_omega, ang->d_solid, 0, ang->spectrum);
+            }
+            ++g_launches;
+            CK(cudaGetLastError());
+            reduced = true;
+        } else if (pl.mode != MODE_DIRECT) {
+            if (pt.kernel == K_SEP) {
+                if (nc == 6) rad_sep_finalize_kernel<6, 2><<<dim3(pl.tiles, 8), SEP_CONS, 0, st>>>(mp);
+                else rad_sep_finalize_kernel<4, 4><<<dim3(pl.tiles, 16), SEP_CONS, 0, st>>>(mp);
+            } else {
+                if (nc == 6) rad_finalize_kernel<6><<<dim3(pl.tiles, W), TPB, 0, st>>>(mp);
+                else rad_finalize_kernel<4><<<dim3(pl.tiles, W), TPB, 0, st>>>(mp);
+            }
+            ++g_launches;
+            CK(cudaGetLastError());
+            reduced = true;
+        }
+    }
+    if (reduced) prof_mark(prof, 3, st);
     return RAD_OK;
 }
 
 static int run_single(const rad_traj *t, const rad_grid *g, int model, double lam, double *out,
-                      void *ws, size_t ws_bytes, cudaStream_t st) {
+                      void *ws, size_t ws_bytes, const rad_options *opt, cudaStream_t st) {
     if (!t) return RAD_EINVAL;
     rad_traj_batch b{1, t->n, nullptr, t->t, t->dz, t->x, t->y, t->vx, t->vy, t->dvz,
                      t->ax, t->ay, t->az, t->gamma};
     const int64_t n = t->n;
-    return run_batch(&b, &n, nullptr, g, model, &lam, 0, out, ws, ws_bytes, st);
+    return run_batch(&b, &n, nullptr, g, model, &lam, 0, out, nullptr, ws, ws_bytes, opt, st);
 }
 
 }  // namespace rad
@@ -733,30 +848,31 @@ using namespace rad;
 extern "C" {
 
 int rad_classical(const rad_traj *traj, const rad_grid *grid, double *out,
-                  void *workspace, size_t workspace_bytes, void *cuda_stream) {
-    return run_single(traj, grid, RAD_CLASSICAL, 0.0, out, workspace, workspace_bytes,
+                  void *workspace, size_t workspace_bytes, const rad_options *opt, void *cuda_stream) {
+    return run_single(traj, grid, RAD_CLASSICAL, 0.0, out, workspace, workspace_bytes, opt,
                       static_cast<cudaStream_t>(cuda_stream));
 }
 
 int rad_semiclassical(const rad_traj *traj, const rad_grid *grid, int spin, double hbarc_over_E,
-                      double *out, void *workspace, size_t workspace_bytes, void *cuda_stream) {
+                      double *out, void *workspace, size_t workspace_bytes, const rad_options *opt,
+                      void *cuda_stream) {
     if (spin != 0 && spin != 1) return RAD_EINVAL;
     if (!(hbarc_over_E >= 0.0)) return RAD_EDOMAIN;
     return run_single(traj, grid, spin == 0 ? RAD_SPIN0 : RAD_SPIN_HALF, hbarc_over_E, out,
-                      workspace, workspace_bytes, static_cast<cudaStream_t>(cuda_stream));
+                      workspace, workspace_bytes, opt, static_cast<cudaStream_t>(cuda_stream));
 }
 
 int rad_ensemble_sum(const rad_traj_batch *batch, const rad_grid *grid, rad_model model,
                      const double *hbarc_over_E, int accumulate, double *out,
-                     void *workspace, size_t workspace_bytes, void *cuda_stream) {
+                     void *workspace, size_t workspace_bytes, const rad_options *opt, void *cuda_stream) {
     if (!batch) return RAD_EINVAL;
-    return run_batch(batch, batch->n, nullptr, grid, (int)model, hbarc_over_E, accumulate, out,
-                     workspace, workspace_bytes, static_cast<cudaStream_t>(cuda_stream));
+    return run_batch(batch, batch->n, nullptr, grid, (int)model, hbarc_over_E, accumulate, out, nullptr,
+                     workspace, workspace_bytes, opt, static_cast<cudaStream_t>(cuda_stream));
 }
 
 int rad_sections_sum(const rad_traj *traj, int32_t n_sections, const int64_t *start, const rad_grid *grid,
                      rad_model model, const double *hbarc_over_E, int accumulate, double *out,
-                     void *workspace, size_t workspace_bytes, void *cuda_stream) {
+                     void *workspace, size_t workspace_bytes, const rad_options *opt, void *cuda_stream) {
     if (!traj || !start || n_sections < 1) return RAD_EINVAL;
     std::vector<int64_t> n(n_sections), off(n_sections);
     for (int s = 0; s < n_sections; ++s) {            // section s = samples start[s] .. start[s+1], both included
@@ -766,8 +882,25 @@ int rad_sections_sum(const rad_traj *traj, int32_t n_sections, const int64_t *st
     }
     rad_traj_batch b{n_sections, traj->n, n.data(), traj->t, traj->dz, traj->x, traj->y, traj->vx, traj->vy,
                      traj->dvz, traj->ax, traj->ay, traj->az, traj->gamma};
-    return run_batch(&b, n.data(), off.data(), grid, (int)model, hbarc_over_E, accumulate, out,
-                     workspace, workspace_bytes, static_cast<cudaStream_t>(cuda_stream));
+    return run_batch(&b, n.data(), off.data(), grid, (int)model, hbarc_over_E, accumulate, out, nullptr,
+                     workspace, workspace_bytes, opt, static_cast<cudaStream_t>(cuda_stream));
+}
+
+int rad_sections_check(int32_t n_sections, const double *t_start, const double *gamma0,
+                       const double *hbarc_over_E, double omega_min, int32_t *short_sections, int32_t cap) {
+    if (n_sections < 1 || !t_start || !gamma0 || cap < 0 || (cap > 0 && !short_sections)) return RAD_EINVAL;
+    if (!(omega_min > 0.0)) return RAD_EDOMAIN;
+    int found = 0;
+    for (int s = 0; s < n_sections; ++s) {
+        if (!(t_start[s + 1] > t_start[s])) return RAD_EINVAL;
+        const double lf = rad_formation_length(gamma0[s], omega_min, hbarc_over_E ? hbarc_over_E[s] : 0.0);
+        if (lf < 0.0) return RAD_EDOMAIN;
+        if (t_start[s + 1] - t_start[s] <= lf) {      // c = 1: a time span is a length
+            if (found < cap) short_sections[found] = s;
+            ++found;
+        }
+    }
+    return found;
 }
 
 int rad_angular_sum(const double *cube, const rad_grid *grid, double d_solid_angle, double theta_cut,
@@ -782,45 +915,72 @@ int rad_angular_sum(const double *cube, const rad_grid *grid, double d_solid_ang
     return RAD_OK;
 }
 
-// omegas per slab of rad_angular_spectrum: the slab cube stays below ~256 MB, whole 16-omega tiles
-static int spectrum_slab(int n_omega, int n_thx, int n_thy) {
-    const int64_t per_omega = (int64_t)n_thx * n_thy * 8;
-    int64_t k = std::max<int64_t>(16, ((int64_t)256 << 20) / per_omega / 16 * 16);
-    return (int)std::min<int64_t>(k, n_omega);
+int rad_number_spectrum(const double *spectrum, const double *omega, int32_t n, double hbar_c, double *number,
+                        void *cuda_stream) {
+    if (!spectrum || !omega || !number || n < 1) return RAD_EINVAL;
+    if (!(hbar_c > 0.0)) return RAD_EDOMAIN;
+    rad_number_spectrum_kernel<<<(n + 255) / 256, 256, 0, static_cast<cudaStream_t>(cuda_stream)>>>(
+        spectrum, omega, n, hbar_c, number);
+    ++g_launches;
+    CK(cudaGetLastError());
+    return RAD_OK;
+}
+
+// Does the angular spectrum of this call come straight out of the main kernel's epilogue?
+static bool angular_is_fused(const CallPlan &cp) { return cp.nparts == 1 && cp.part[0].plan.mode == MODE_DIRECT && !cp.fused; }
+
+static size_t angular_workspace(int count, int64_t n_max, int n_omega, int n_thx, int n_thy) {
+    size_t need = 0;
+    bool all_fused = true;
+    for (int kernel = 0; kernel <= 2; ++kernel)
+        for (int nc = 4; nc <= 6; nc += 2) {
+            const CallPlan cp = plan_for(count, n_max, n_omega, n_thx, n_thy, nc, kernel, true);
+            if (angular_is_fused(cp)) need = std::max(need, cp.total);
+            else all_fused = false;
+        }
+    if (!all_fused)           // cube path (grids of fewer than 8 tiles per SM): the call's own workspace + the cube
+        need = std::max(need, align_up(rad_workspace_bytes(count, n_max, n_omega, n_thx, n_thy), 256)
+                                  + align_up((size_t)n_omega * n_thx * n_thy * 8, 256));
+    return need;
 }
 
 size_t rad_angular_spectrum_workspace_bytes(int32_t count, int64_t n_max, int32_t n_omega, int32_t n_thx,
                                             int32_t n_thy) {
     if (count < 1 || n_max < 2 || n_omega < 1 || n_thx < 1 || n_thy < 1) return 0;
-    const int k = spectrum_slab(n_omega, n_thx, n_thy);
-    const size_t inner = rad_workspace_bytes(count, n_max, k, n_thx, n_thy);
-    return align_up(inner, 256) + align_up((size_t)k * n_thx * n_thy * 8, 256);
+    return angular_workspace(count, n_max, n_omega, n_thx, n_thy);
 }
 
 int rad_angular_spectrum(const rad_traj_batch *batch, const rad_grid *grid, rad_model model,
                          const double *hbarc_over_E, double d_solid_angle, double theta_cut, double *spectrum,
-                         void *workspace, size_t workspace_bytes, void *cuda_stream) {
+                         void *workspace, size_t workspace_bytes, const rad_options *opt, void *cuda_stream) {
     if (!batch || !grid_ok(grid) || !spectrum || !workspace) return RAD_EINVAL;
     if (reinterpret_cast<uintptr_t>(workspace) & 255) return RAD_EINVAL;
+    if (model < RAD_CLASSICAL || model > RAD_SPIN_HALF) return RAD_EINVAL;
     int64_t n_max = 0;
     if (!batch->n || batch->count < 1) return RAD_EINVAL;
     for (int p = 0; p < batch->count; ++p) n_max = std::max(n_max, batch->n[p]);
     if (n_max < 2) return RAD_EINVAL;
-    const int k = spectrum_slab(grid->n_omega, grid->n_thx, grid->n_thy);
-    const size_t inner = align_up(rad_workspace_bytes(batch->count, n_max, k, grid->n_thx, grid->n_thy), 256);
-    const size_t cube_bytes = align_up((size_t)k * grid->n_thx * grid->n_thy * 8, 256);
+    const int kopt = kernel_option(opt);
+    if (kopt < RAD_KERNEL_AUTO || kopt > RAD_KERNEL_SEPARABLE) return RAD_EINVAL;
+    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
+    const int nc = model == RAD_SPIN_HALF ? 6 : 4;
+    const double cut2 = theta_cut > 0.0 ? theta_cut * theta_cut : 0.0;
+    const CallPlan cp = plan_for(batch->count, n_max, grid->n_omega, grid->n_thx, grid->n_thy, nc, kopt, true);
+    if (angular_is_fused(cp)) {                       // no cube: sums formed in the main kernel's epilogue
+        if (workspace_bytes < cp.total) return RAD_ENOSPACE;
+        const AngularOut ang{d_solid_angle, cut2, spectrum};
+        return run_batch(batch, batch->n, nullptr, grid, (int)model, hbarc_over_E, 0, nullptr, &ang,
+                         workspace, workspace_bytes, opt, st);
+    }
+    // small grid (fewer than 8 tiles per SM, i.e. a cube below 40 MB): the cube inside the workspace, then its sum
+    const size_t inner = align_up(rad_workspace_bytes(batch->count, n_max, grid->n_omega, grid->n_thx, grid->n_thy), 256);
+    const size_t cube_bytes = align_up((size_t)grid->n_omega * grid->n_thx * grid->n_thy * 8, 256);
     if (workspace_bytes < inner + cube_bytes) return RAD_ENOSPACE;
     double *cube = reinterpret_cast<double *>(static_cast<char *>(workspace) + inner);
-    cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
-    for (int w0 = 0; w0 < grid->n_omega; w0 += k) {    // one slab of omegas at a time: cube of the slab, then its sum
-        const int kw = std::min(k, grid->n_omega - w0);
-        rad_grid slab{kw, grid->n_thx, grid->n_thy, grid->omega + w0, grid->thx, grid->thy};
-        int rc = run_batch(batch, batch->n, nullptr, &slab, (int)model, hbarc_over_E, 0, cube, workspace, inner, st);
-        if (rc != RAD_OK) return rc;
-        rc = rad_angular_sum(cube, &slab, d_solid_angle, theta_cut, spectrum + w0, cuda_stream);
-        if (rc != RAD_OK) return rc;
-    }
-    return RAD_OK;
+    const int rc = run_batch(batch, batch->n, nullptr, grid, (int)model, hbarc_over_E, 0, cube, nullptr,
+                             workspace, inner, opt, st);
+    if (rc != RAD_OK) return rc;
+    return rad_angular_sum(cube, grid, d_solid_angle, theta_cut, spectrum, cuda_stream);
 }
 
 int rad_generate_trajectories(rad_well well, double kappa, double length, double gamma, double dt,
@@ -862,15 +1022,16 @@ int rad_sum_cubes(const double *cubes, int32_t count, int64_t m, int accumulate,
 size_t rad_workspace_bytes(int32_t count, int64_t n_max, int32_t n_omega, int32_t n_thx, int32_t n_thy) {
     if (count < 1 || n_max < 2 || n_omega < 1 || n_thx < 1 || n_thy < 1) return 0;
     size_t need = 0;                                   // whichever kernel and variant the call ends up using
-    for (int kernel = 0; kernel < 2; ++kernel)
+    for (int kernel = 0; kernel <= 3; ++kernel)
         for (int nc = 4; nc <= 6; nc += 2)
-            need = std::max(need, make_plan(count, n_max, n_omega, n_thx, n_thy, nc, kernel).total);
+            need = std::max(need, plan_for(count, n_max, n_omega, n_thx, n_thy, nc, kernel, false).total);
     return need;
 }
 
 // ---- host-buffer variants: H2D once, compute, D2H once
 int rad_ensemble_sum_host(const rad_traj_batch *b, const rad_grid *g, rad_model model,
-                          const double *hbarc_over_E, int accumulate, double *out, void *cuda_stream) {
+                          const double *hbarc_over_E, int accumulate, double *out, const rad_options *opt,
+                          void *cuda_stream) {
     if (!b || b->count < 1 || !b->n || !grid_ok(g) || !out) return RAD_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const size_t row = (size_t)b->stride, tot = row * b->count;
@@ -880,7 +1041,7 @@ int rad_ensemble_sum_host(const rad_traj_batch *b, const rad_grid *g, rad_model 
     for (const double *p : src)
         if (!p) return RAD_EINVAL;
     double *dev = nullptr;
-    CK(cudaMallocAsync(reinterpret_cast<void **>(&dev), (11 * tot + ng + M) * sizeof(double), st));
+    CK(pool_alloc(reinterpret_cast<void **>(&dev), (11 * tot + ng + M) * sizeof(double), st));
     PoolScratch pool;
     pool.p = dev; pool.st = st;
     const double *d[11];
@@ -895,7 +1056,7 @@ int rad_ensemble_sum_host(const rad_traj_batch *b, const rad_grid *g, rad_model 
     if (accumulate) CK(cudaMemcpyAsync(dout, out, M * sizeof(double), cudaMemcpyHostToDevice, st));
     rad_traj_batch db{b->count, b->stride, b->n, d[0], d[1], d[2], d[3], d[4], d[5], d[6], d[7], d[8], d[9], d[10]};
     rad_grid dg{g->n_omega, g->n_thx, g->n_thy, gw, gx, gy};
-    int rc = run_batch(&db, b->n, nullptr, &dg, (int)model, hbarc_over_E, accumulate, dout, nullptr, 0, st);
+    int rc = run_batch(&db, b->n, nullptr, &dg, (int)model, hbarc_over_E, accumulate, dout, nullptr, nullptr, 0, opt, st);
     if (rc == RAD_OK) {
         cudaError_t e = cudaMemcpyAsync(out, dout, M * sizeof(double), cudaMemcpyDeviceToHost, st);
         if (e != cudaSuccess) rc = cuda_fail(e, "D2H");
@@ -908,12 +1069,12 @@ int rad_ensemble_sum_host(const rad_traj_batch *b, const rad_grid *g, rad_model 
 }
 
 int rad_eval_host(const rad_traj *t, const rad_grid *g, rad_model model, double hbarc_over_E,
-                  double *out, void *cuda_stream) {
+                  double *out, const rad_options *opt, void *cuda_stream) {
     if (!t) return RAD_EINVAL;
     if (model != RAD_CLASSICAL && !(hbarc_over_E >= 0.0)) return RAD_EDOMAIN;
     const int64_t n = t->n;
     rad_traj_batch b{1, t->n, &n, t->t, t->dz, t->x, t->y, t->vx, t->vy, t->dvz, t->ax, t->ay, t->az, t->gamma};
-    return rad_ensemble_sum_host(&b, g, model, &hbarc_over_E, 0, out, cuda_stream);
+    return rad_ensemble_sum_host(&b, g, model, &hbarc_over_E, 0, out, opt, cuda_stream);
 }
 
 double rad_measure_fp64_peak(double millis, void *cuda_stream) {
@@ -951,9 +1112,16 @@ double rad_measure_fp64_peak(double millis, void *cuda_stream) {
 
 int64_t rad_launch_count(void) { return g_launches.load(); }
 
-int rad_plan_kernel(int32_t n_omega, int32_t n_thx, int32_t n_thy, rad_model model) {
-    if (n_omega < 1 || n_thx < 1 || n_thy < 1 || model < RAD_CLASSICAL || model > RAD_SPIN_HALF) return RAD_EINVAL;
-    return choose_kernel(n_omega, n_thx, n_thy, model == RAD_SPIN_HALF ? 6 : 4) + 1;
+static int kernel_code(const CallPlan &cp) { return cp.fused ? 3 : cp.part[0].kernel == K_SEP ? 2 : 1; }
+
+int rad_plan_kernel(int32_t count, int64_t n_max, int32_t n_omega, int32_t n_thx, int32_t n_thy,
+                    rad_model model, int32_t kernel) {
+    if (count < 1 || n_max < 2 || n_omega < 1 || n_thx < 1 || n_thy < 1) return RAD_EINVAL;
+    if (model < RAD_CLASSICAL || model > RAD_SPIN_HALF || kernel < 0 || kernel > 3) return RAD_EINVAL;
+    const int nc = model == RAD_SPIN_HALF ? 6 : 4;
+    const CallPlan cp = plan_for(count, n_max, n_omega, n_thx, n_thy, nc, kernel, false);
+    if (kernel == 3 && !cp.fused) return RAD_EINVAL;
+    return kernel_code(cp);
 }
 
 double rad_formation_length(double gamma, double omega, double hbarc_over_E) {
@@ -963,40 +1131,52 @@ double rad_formation_length(double gamma, double omega, double hbarc_over_E) {
 }
 
 int rad_plan_describe(int32_t count, int64_t n_max, int32_t n_omega, int32_t n_thx, int32_t n_thy, rad_model model,
-                      int32_t *plan) {
+                      int32_t kernel, int32_t *plan) {
     if (!plan || count < 1 || n_max < 2 || n_omega < 1 || n_thx < 1 || n_thy < 1) return RAD_EINVAL;
-    if (model < RAD_CLASSICAL || model > RAD_SPIN_HALF) return RAD_EINVAL;
+    if (model < RAD_CLASSICAL || model > RAD_SPIN_HALF || kernel < 0 || kernel > 3) return RAD_EINVAL;
     const int nc = model == RAD_SPIN_HALF ? 6 : 4;
-    const Plan pl = make_plan(count, n_max, n_omega, n_thx, n_thy, nc, choose_kernel(n_omega, n_thx, n_thy, nc));
-    plan[0] = pl.kernel + 1;
-    plan[1] = pl.mode;
-    plan[2] = pl.tiles;
-    plan[3] = pl.mode == MODE_TSPLIT ? count * pl.t_slices : pl.p_slices;      // gridDim.y
-    plan[4] = pl.t_slices;
-    plan[5] = pl.cpt;
+    const CallPlan cp = plan_for(count, n_max, n_omega, n_thx, n_thy, nc, kernel, false);
+    if (kernel == 3 && !cp.fused) return RAD_EINVAL;
+    const Plan &pl = cp.part[0].plan;
+    plan[0] = kernel_code(cp);
+    plan[1] = cp.fused ? MODE_TSPLIT : pl.mode;
+    plan[2] = cp.fused ? cp.fused_tiles : pl.tiles;
+    plan[3] = cp.fused ? cp.fused_slices : pl.slices();
+    plan[4] = cp.fused ? cp.fused_slices : pl.t_slices;
+    plan[5] = cp.cpt;
+    plan[6] = cp.fused ? 1 : cp.nparts;
+    plan[7] = !cp.fused && cp.nparts == 2 ? cp.part[0].n_thx : 0;
+    plan[8] = !cp.fused && cp.nparts == 2 ? cp.part[0].n_thy : 0;
+    plan[9] = cp.launches();
     return RAD_OK;
 }
 
-int rad_set_kernel(int choice) {
-    if (choice < 0 || choice > 2) return RAD_EINVAL;
-    g_kernel_choice.store(choice);
-    return RAD_OK;
+rad_profile *rad_profile_create(void) {
+    rad_profile *p = new (std::nothrow) rad_profile{};
+    if (!p) return nullptr;
+    for (int i = 0; i < 4; ++i)
+        if (cudaEventCreate(&p->ev[i]) != cudaSuccess) {
+            cudaGetLastError();
+            for (int k = 0; k < i; ++k) cudaEventDestroy(p->ev[k]);
+            delete p;
+            return nullptr;
+        }
+    return p;
 }
 
-int rad_profile_enable(int on) {
-    g_prof.store(on ? 1 : 0);
-    return RAD_OK;
+void rad_profile_destroy(rad_profile *p) {
+    if (!p) return;
+    for (auto &e : p->ev) cudaEventDestroy(e);
+    delete p;
 }
 
-int rad_profile_last(float *ms) {
-    if (!ms) return RAD_EINVAL;
-    std::lock_guard<std::mutex> lk(g_ev_mu);
-    if (!g_ev_ready) return RAD_EINVAL;
-    CK(cudaEventSynchronize(g_ev[g_ev_have_finalize ? 3 : 2]));
-    CK(cudaEventElapsedTime(&ms[0], g_ev[0], g_ev[1]));
-    CK(cudaEventElapsedTime(&ms[1], g_ev[1], g_ev[2]));
+int rad_profile_read(rad_profile *p, float *ms) {
+    if (!p || !ms) return RAD_EINVAL;
+    CK(cudaEventSynchronize(p->ev[p->have_reduce ? 3 : 2]));
+    CK(cudaEventElapsedTime(&ms[0], p->ev[0], p->ev[1]));
+    CK(cudaEventElapsedTime(&ms[1], p->ev[1], p->ev[2]));
     ms[2] = 0.f;
-    if (g_ev_have_finalize) CK(cudaEventElapsedTime(&ms[2], g_ev[2], g_ev[3]));
+    if (p->have_reduce) CK(cudaEventElapsedTime(&ms[2], p->ev[2], p->ev[3]));
     return RAD_OK;
 }
 

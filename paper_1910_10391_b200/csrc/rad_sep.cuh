@@ -400,15 +400,16 @@ rad_sep_kernel(const MainParams P) {
     const int rF = co.wx * 2 * WY * 16 + co.lx * 4 + co.ly;               // + (j*WY + m) * 16
 
     // ---- output slots of this thread: zero them, later every trajectory adds its spectrum
-    const int A = P.n_thx * P.n_thy;
     auto out_slot = [&](int e) -> double * {          // nullptr: point outside the grid
         const int m = e % WY, j = (e / WY) & 1, i = e / (2 * WY);
         const int iw = co.iw0 + i, ix = co.ix0 + j, iy = co.iy0 + m;
         if (P.mode == MODE_PSLICE) return P.partial + ((int64_t)slice * EV + e) * P.t_pad + gid;
         if (iw >= P.n_omega || ix >= P.n_thx || iy >= P.n_thy) return nullptr;
-        return P.out + (int64_t)iw * A + (int64_t)iy * P.n_thx + ix;
+        return P.out + iw * P.out_plane + (int64_t)iy * P.out_nx + ix;
     };
-    if (P.mode != MODE_TSPLIT && !(P.mode == MODE_DIRECT && P.accumulate)) {
+    const bool ang = P.mode == MODE_DIRECT && P.ang;
+    double sw[2] = {0.0, 0.0};                        // angular spectrum: this thread's angles summed, per omega (N1)
+    if (P.mode != MODE_TSPLIT && !(P.mode == MODE_DIRECT && P.accumulate) && !ang) {
 #pragma unroll 1
         for (int e = 0; e < EV; ++e) {
             double *o = out_slot(e);
@@ -518,8 +519,15 @@ rad_sep_kernel(const MainParams P) {
                     const double om = P.omega[min(co.iw0 + i, P.n_omega - 1)];
                     const double nx = P.thx[min(co.ix0 + j, P.n_thx - 1)];
                     const double ny = P.thy[min(co.iy0 + m, P.n_thy - 1)];
-                    double *o = out_slot(e);
-                    if (o) *o += spectrum_value_true<NC>(acc[e], nx, ny, P.model, om * lam, gamma0);
+                    const double v = spectrum_value_true<NC>(acc[e], nx, ny, P.model, om * lam, gamma0);
+                    if (ang) {
+                        const bool inside = co.iw0 + i < P.n_omega && co.ix0 + j < P.n_thx && co.iy0 + m < P.n_thy
+                                            && (P.cut2 <= 0.0 || fma(nx, nx, ny * ny) <= P.cut2);
+                        if (inside) sw[i] += v;
+                    } else {
+                        double *o = out_slot(e);
+                        if (o) *o += v;
+                    }
                 }
             }
 #pragma unroll
@@ -532,6 +540,43 @@ rad_sep_kernel(const MainParams P) {
             } while (p_now < p_end && todo == 0);
         }
     }
+    if (ang) {
+        // ---- sum over the tile's angles per omega, fixed order: 16 omega slots (slot = i_w - bw = 4 ww + 2 lw + i),
+        // each fed by the 32 consumer threads (2 warps x 16 lanes) that own that omega.  The trajectory ring is
+        // free by now: every chunk was consumed before the last table block was handed over.
+        asm volatile("bar.sync 2, 256;" ::: "memory");
+        double *red = ring;                           // [256][2]
+        red[tid * 2] = sw[0]; red[tid * 2 + 1] = sw[1];
+        asm volatile("bar.sync 2, 256;" ::: "memory");
+        if (tid < 16) {
+            const int ww = tid >> 2, lw = (tid >> 1) & 1, i = tid & 1;
+            double sum = 0.0;
+            for (int wx = 0; wx < 2; ++wx)
+                for (int l = 0; l < 16; ++l) sum += red[(((ww * 2 + wx) * 32) + l * 2 + lw) * 2 + i];
+            P.ang_partial[(int64_t)blockIdx.x * 16 + tid] = sum;
+        }
+    }
+}
+
+// angular spectrum, second pass for the separable kernel: spec[i_w] (+)= d_solid * sum over the angle tiles of
+// omega tile i_w / 16 (contiguous block indices), ascending; one CTA per omega, fixed two-level order.
+__global__ void __launch_bounds__(256)
+rad_ang_final_sep_kernel(const double *partial, int angle_tiles, int n_omega, double d_solid, int accumulate,
+                         double *spec) {
+    __shared__ double red[256];
+    const int iw = blockIdx.x, wt = iw / 16, slot = iw % 16;
+    const int per = (angle_tiles + 255) / 256;
+    double s = 0.0;
+    for (int t = threadIdx.x * per; t < min(angle_tiles, (threadIdx.x + 1) * per); ++t)
+        s += partial[((int64_t)wt * angle_tiles + t) * 16 + slot];
+    red[threadIdx.x] = s;
+    __syncthreads();
+    if (threadIdx.x == 0) {
+        double tot = 0.0;
+        for (int k = 0; k < 256; ++k) tot += red[k];
+        tot *= d_solid;
+        spec[iw] = accumulate ? spec[iw] + tot : tot;
+    }
 }
 
 // ------------------------------------------------------------------------------ finalize (a6, a7)
@@ -541,7 +586,6 @@ rad_sep_finalize_kernel(const MainParams P) {
     constexpr int EV = 4 * WY;
     const SepCoord<WY> co(blockIdx.x, threadIdx.x, P.n_thx, P.n_thy);
     const int64_t gid = (int64_t)blockIdx.x * SEP_CONS + threadIdx.x;
-    const int A = P.n_thx * P.n_thy;
     {                                                 // gridDim.y = EV: one of the thread's points per CTA row
         const int e = blockIdx.y;
         const int m = e % WY, j = (e / WY) & 1, i = e / (2 * WY);
@@ -567,7 +611,7 @@ rad_sep_finalize_kernel(const MainParams P) {
                 total += spectrum_value_true<NC>(acc, nx, ny, P.model, om * lam, gamma0);
             }
         }
-        double *o = P.out + (int64_t)iw * A + (int64_t)iy * P.n_thx + ix;
+        double *o = P.out + iw * P.out_plane + (int64_t)iy * P.out_nx + ix;
         *o = P.accumulate ? *o + total : total;
     }
 }

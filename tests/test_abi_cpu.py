@@ -68,33 +68,40 @@ def test_validation_happens_before_any_cuda_call(radlib):
     grid = B._Grid(2, 2, 2, p, p, p)
     traj = B._Traj(8, *([p] * 11))
     out = np.zeros(8).ctypes.data
-    assert lib.rad_classical(None, ctypes.byref(grid), out, None, 0, None) == -1
-    assert lib.rad_classical(ctypes.byref(traj), None, out, None, 0, None) == -1
-    assert lib.rad_classical(ctypes.byref(traj), ctypes.byref(grid), None, None, 0, None) == -1
-    assert lib.rad_semiclassical(ctypes.byref(traj), ctypes.byref(grid), 3, 1e-15, out, None, 0, None) == -1
-    assert lib.rad_semiclassical(ctypes.byref(traj), ctypes.byref(grid), 1, -1.0, out, None, 0, None) == -2
-    assert lib.rad_classical(ctypes.byref(B._Traj(1, *([p] * 11))), ctypes.byref(grid), out, None, 0, None) == -1
+    assert lib.rad_classical(None, ctypes.byref(grid), out, None, 0, None, None) == -1
+    assert lib.rad_classical(ctypes.byref(traj), None, out, None, 0, None, None) == -1
+    assert lib.rad_classical(ctypes.byref(traj), ctypes.byref(grid), None, None, 0, None, None) == -1
+    assert lib.rad_semiclassical(ctypes.byref(traj), ctypes.byref(grid), 3, 1e-15, out, None, 0, None, None) == -1
+    assert lib.rad_semiclassical(ctypes.byref(traj), ctypes.byref(grid), 1, -1.0, out, None, 0, None, None) == -2
+    assert lib.rad_classical(ctypes.byref(B._Traj(1, *([p] * 11))), ctypes.byref(grid), out, None, 0, None, None) == -1
     assert lib.rad_classical(ctypes.byref(B._Traj(8, *([p] * 10 + [None]))), ctypes.byref(grid), out,
-                             None, 0, None) == -1
-    assert lib.rad_classical(ctypes.byref(traj), ctypes.byref(B._Grid(0, 2, 2, p, p, p)), out, None, 0, None) == -1
+                             None, 0, None, None) == -1
+    assert lib.rad_classical(ctypes.byref(traj), ctypes.byref(B._Grid(0, 2, 2, p, p, p)), out, None, 0, None, None) == -1
     misaligned = B._Traj(8, *([p + 4] + [p] * 10))
-    assert lib.rad_classical(ctypes.byref(misaligned), ctypes.byref(grid), out, None, 0, None) == -1
+    assert lib.rad_classical(ctypes.byref(misaligned), ctypes.byref(grid), out, None, 0, None, None) == -1
     n = np.array([8, 1], dtype=np.int64)
     batch = B._Batch(2, 8, n.ctypes.data, *([p] * 11))
-    assert lib.rad_ensemble_sum(ctypes.byref(batch), ctypes.byref(grid), 0, None, 0, out, None, 0, None) == -1
+    assert lib.rad_ensemble_sum(ctypes.byref(batch), ctypes.byref(grid), 0, None, 0, out, None, 0, None, None) == -1
     n[1] = 9                                                          # n[p] > stride
-    assert lib.rad_ensemble_sum(ctypes.byref(batch), ctypes.byref(grid), 0, None, 0, out, None, 0, None) == -1
+    assert lib.rad_ensemble_sum(ctypes.byref(batch), ctypes.byref(grid), 0, None, 0, out, None, 0, None, None) == -1
     n[1] = 8
-    assert lib.rad_ensemble_sum(ctypes.byref(batch), ctypes.byref(grid), 2, None, 0, out, None, 0, None) == -1
+    assert lib.rad_ensemble_sum(ctypes.byref(batch), ctypes.byref(grid), 2, None, 0, out, None, 0, None, None) == -1
     assert lib.rad_angular_sum(None, ctypes.byref(grid), 1.0, 0.0, out, None) == -1
     start = np.array([0, 4, 4], dtype=np.int64)                       # empty section
     assert lib.rad_sections_sum(ctypes.byref(traj), 2, start.ctypes.data, ctypes.byref(grid), 0, None, 0, out,
-                                None, 0, None) == -1
+                                None, 0, None, None) == -1
     start = np.array([0, 4, 8], dtype=np.int64)                       # runs past the last sample (n = 8)
     assert lib.rad_sections_sum(ctypes.byref(traj), 2, start.ctypes.data, ctypes.byref(grid), 0, None, 0, out,
-                                None, 0, None) == -1
+                                None, 0, None, None) == -1
     assert lib.rad_sections_sum(ctypes.byref(traj), 0, start.ctypes.data, ctypes.byref(grid), 0, None, 0, out,
-                                None, 0, None) == -1
+                                None, 0, None, None) == -1
+    bad = B._Options(9, 0, None)                                      # unknown kernel option; reserved must be 0
+    assert lib.rad_classical(ctypes.byref(traj), ctypes.byref(grid), out, None, 0, ctypes.byref(bad), None) == -1
+    bad = B._Options(0, 1, None)
+    assert lib.rad_classical(ctypes.byref(traj), ctypes.byref(grid), out, None, 0, ctypes.byref(bad), None) == -1
+    fused = B._Options(3, 0, None)                                    # fused kernel: single trajectory only
+    assert lib.rad_ensemble_sum(ctypes.byref(batch), ctypes.byref(grid), 0, None, 0, out, None, 0,
+                                ctypes.byref(fused), None) == -1
 
 
 def test_no_cpu_fallback(radlib):
@@ -114,28 +121,36 @@ def test_no_cpu_fallback(radlib):
 
 def test_kernel_choice_is_a_pure_function_of_the_shape(radlib):
     """rad_plan_kernel without a device: separable kernel where the grid fills its 16 x 16 x 16 (8) point
-    tiles (BASELINE.json configs 2-5), direct kernel on small angle grids (config 1)."""
+    tiles (BASELINE.json configs 2-5), direct kernel on small angle grids with long trajectories, the fused
+    single-launch kernel on small problems (config 1); the per-call option overrides."""
     f = radlib.rad_plan_kernel
     assert f(256, 32, 32, 0) == 2 and f(512, 64, 64, 2) == 2 and f(128, 16, 16, 0) == 2 and f(1024, 64, 64, 1) == 2
-    assert f(64, 8, 8, 0) == 1 and f(5, 3, 3, 2) == 1
-    radlib.rad_set_kernel(1)
-    assert f(256, 32, 32, 0) == 1
-    radlib.rad_set_kernel(0)
+    assert f(64, 8, 8, 0) == 1 and f(5, 3, 3, 2) == 1                 # n_max defaults to 2^20: too long to fuse
+    assert f(64, 8, 8, 0, n_max=4000) == 3                            # BASELINE config 1
+    assert f(64, 8, 8, 0, n_max=4000, count=3) == 1                   # ensembles are never fused
+    assert f(256, 32, 32, 0, kernel=1) == 1 and f(64, 8, 8, 0, kernel=2) == 2
+    assert f(64, 8, 8, 2, kernel=3, n_max=100000) == 3                # forced: any single trajectory that fits
     with pytest.raises(radlib.RadError):
         f(0, 4, 4, 0)
+    with pytest.raises(radlib.RadError):
+        f(1024, 64, 64, 0, kernel=3)                                  # more tiles than the GPU holds at once
 
 
 def test_launch_plans_of_the_baseline_configs(radlib):
     """The plan is host logic: a pure function of the shapes (148 SMs assumed without a device).  The five
-    BASELINE.json configs get whole waves of CTAs: separable kernel 1 CTA/SM, direct kernel 2 CTAs/SM."""
+    BASELINE.json configs get whole waves of CTAs: separable kernel 1 CTA/SM, direct kernel 2 CTAs/SM, fused
+    kernel 4 CTAs/SM all resident at once."""
     import torch
     if torch.cuda.is_available():
         pytest.skip("plan depends on the visible device's SM count; this checks the 148-SM default")
     d = radlib.rad_plan_describe
-    p = d(1, 4000, 64, 8, 8, 0)                      # cfg 1: direct kernel, 4 tiles x 32 one-chunk time slices
-    assert (p["kernel"], p["mode"], p["tiles"], p["slices"], p["chunks"]) == (1, 2, 4, 32, 32)
+    p = d(1, 4000, 64, 8, 8, 0)                      # cfg 1: fused kernel, 8 tiles of 64 threads x 62 time slices, ONE launch
+    assert (p["kernel"], p["tiles"], p["slices"], p["launches"]) == (3, 8, 62, 1)
+    assert p["tiles"] * p["slices"] <= 4 * 148
+    p = d(1, 4000, 64, 8, 8, 0, kernel=1)            # the three-launch direct path: 4 tiles x 32 one-chunk time slices
+    assert (p["kernel"], p["mode"], p["tiles"], p["slices"], p["chunks"], p["launches"]) == (1, 2, 4, 32, 32, 3)
     p = d(1, 14287, 256, 32, 32, 0)                  # cfg 2: 64 tiles x 16 time slices = 6.92 waves of 148
-    assert (p["kernel"], p["mode"], p["tiles"], p["slices"]) == (2, 2, 64, 16)
+    assert (p["kernel"], p["mode"], p["tiles"], p["slices"], p["parts"]) == (2, 2, 64, 16, 1)
     p = d(1, 200000, 512, 64, 64, 2)                 # cfg 3 spin-1/2: 16 x 16 x 8 point tiles -> 1024 CTAs = 6.92 waves
     assert (p["kernel"], p["mode"], p["tiles"], p["slices"]) == (2, 0, 1024, 1)
     p = d(1, 200000, 512, 64, 64, 1)                 # cfg 3 spin-0: 16 x 16 x 16 tiles -> 512 tiles x 2 time slices
@@ -145,16 +160,65 @@ def test_launch_plans_of_the_baseline_configs(radlib):
     p = d(1, 1000000, 1024, 64, 64, 1)               # cfg 5 spin-0: 1024 tiles, one CTA per tile
     assert (p["kernel"], p["mode"], p["tiles"], p["slices"]) == (2, 0, 1024, 1)
     p = d(1, 1000000, 1024, 64, 64, 2)               # cfg 5 spin-1/2: 2048 tiles = 13.8 waves
-    assert (p["kernel"], p["mode"], p["tiles"], p["slices"]) == (2, 0, 2048, 1)
-    radlib.rad_set_kernel(1)
-    try:
-        p = d(1, 14287, 256, 32, 32, 0)              # direct kernel on cfg 2: 256 tiles x 8 = 6.92 waves of 296
-        assert (p["kernel"], p["mode"], p["tiles"], p["slices"]) == (1, 2, 256, 8)
-    finally:
-        radlib.rad_set_kernel(0)
+    assert (p["kernel"], p["mode"], p["tiles"], p["slices"], p["launches"]) == (2, 0, 2048, 1, 2)
+    p = d(1, 14287, 256, 32, 32, 0, kernel=1)        # direct kernel on cfg 2: 256 tiles x 8 = 6.92 waves of 296
+    assert (p["kernel"], p["mode"], p["tiles"], p["slices"]) == (1, 2, 256, 8)
     for k in range(1, 60):                           # slices never exceed the work there is
         p = d(k, 300, 16, 16, 16, 0)
         assert p["slices"] <= k * p["chunks"] and p["slices"] >= 1
+
+
+def test_the_papers_typical_grid_is_split_in_two_parts(radlib):
+    """N_x = N_y = 50, N_w = 100 "when multiple scattering is included".  50 is 3 tiles of 16 + 2:
+    the separable kernel takes the 48 x 48 interior (63 tiles for 100 -> 112 omegas, 441 CTAs = 2.98 waves), the
+    direct kernel the L-shaped rest of 196 angles; padding to 64 x 64 (fill 0.55) or the direct kernel alone
+    would both be slower.  Grids that fill whole tiles, and small problems, stay in one part."""
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("plan depends on the visible device's SM count; this checks the 148-SM default")
+    d = radlib.rad_plan_describe
+    p = d(1, 3000, 100, 50, 50, 0)
+    assert (p["kernel"], p["parts"], p["interior_x"], p["interior_y"], p["tiles"], p["slices"]) == (2, 2, 48, 48, 63, 7)
+    assert p["launches"] == 5                         # pack, separable main + reduction, direct main + reduction
+    p = d(1, 3000, 100, 50, 50, 2)                   # spin-1/2: 16 x 16 x 8 tiles, 48 = 6 x 8 rows
+    assert (p["parts"], p["interior_x"], p["interior_y"]) == (2, 48, 48)
+    assert d(1, 14287, 256, 32, 32, 0)["parts"] == 1 and d(1, 3000, 100, 64, 48, 0)["parts"] == 1
+    assert d(1, 3000, 100, 60, 60, 0)["parts"] == 1  # remainder 12 of 16: padding is cheaper than a second launch
+    p = d(1, 3000, 100, 50, 64, 0)                   # only the x axis leaves a rest
+    assert (p["parts"], p["interior_x"], p["interior_y"]) == (2, 48, 64)
+    assert d(1, 3000, 17, 17, 17, 0)["kernel"] == 3  # 1.5e7 evals: the fused single-launch kernel
+
+
+def test_sections_check(radlib):
+    """every section must be longer than the formation length l_f = 2 gamma^2 (E - w)/(E w) at the
+    lowest frequency of interest.  Golden numbers: the paper's own example (50 GeV, 5 GeV photon: 680 nm by the
+    formula) and its 0.1 mm sections."""
+    rows = [ln.split() for ln in (ROOT / "tests" / "golden" / "formation_length.txt").read_text().splitlines()
+            if ln and not ln.startswith("#")]
+    E_eV, w_eV, formula_m, _ = (float(v) for v in rows[0])
+    me, hbarc = 0.51099895e6, 1.973269804e-7
+    gamma, omega, lam = E_eV / me, w_eV / hbarc, hbarc / E_eV
+    # boundaries: 0.1 mm sections (PAPER.md:75) and two short ones, just below and just above l_f
+    t = np.array([0.0, 1e-4, 1e-4 + 0.999 * formula_m, 2e-4, 2e-4 + 1.001 * formula_m, 3e-4])
+    g = np.full(5, gamma)
+    assert list(radlib.rad_sections_check(t, g, omega, lam)) == [1]
+    # classical (no recoil): l_f = 2 gamma^2 / w is longer by E/(E - w) = 1/0.9 -> section 3 is now too short as well
+    assert list(radlib.rad_sections_check(t, g, omega)) == [1, 3]
+    # a lower frequency lengthens l_f ~ 1/w: at w/1000 the 0.1 mm sections themselves are too short
+    assert list(radlib.rad_sections_check(t, g, omega / 1000, lam)) == [0, 1, 2, 3, 4]
+    # per-section energy: halving gamma quarters l_f
+    g2 = g.copy()
+    g2[1] = gamma / 2
+    assert list(radlib.rad_sections_check(t, g2, omega, lam * np.array([1, 2, 1, 1, 1]))) == []
+    with pytest.raises(radlib.RadError):
+        radlib.rad_sections_check(t, g, 0.0, lam)                     # omega_min must be positive
+    with pytest.raises(radlib.RadError):
+        radlib.rad_sections_check(t[::-1].copy(), g, omega, lam)      # boundaries must ascend
+    lib = radlib.load_library()                                       # raw ABI: count returned even when cap is too small
+    idx = np.zeros(1, dtype=np.int32)
+    lamv = np.full(5, lam)
+    assert lib.rad_sections_check(5, t.ctypes.data, g.ctypes.data, lamv.ctypes.data, omega / 1000, idx.ctypes.data, 1) == 5
+    assert idx[0] == 0
 
 
 def test_formation_length_of_the_papers_example(radlib):

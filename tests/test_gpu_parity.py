@@ -57,11 +57,12 @@ def assert_parity(gpu_cube, ref, idx=None, label=""):
     return float(ratio[worst])
 
 
-def run_single(rad, wl, model, lam):
+def run_single(rad, wl, model, lam, kernel=0):
+    """kernel: rad_options.kernel of the call (0 auto, 1 direct, 2 separable, 3 fused single-launch)."""
     tr, g = dev_dict(wl.traj), dev_grid(wl)
     if model == CL:
-        return rad.rad_classical(tr, *g).cpu().numpy()
-    return rad.rad_semiclassical(tr, *g, 0 if model == S0 else 1, lam).cpu().numpy()
+        return rad.rad_classical(tr, *g, kernel=kernel).cpu().numpy()
+    return rad.rad_semiclassical(tr, *g, 0 if model == S0 else 1, lam, kernel=kernel).cpu().numpy()
 
 
 def sampled_reference(oracle_mod, wl, cube, n_random, lattice, model, lam, seed=1):
@@ -151,11 +152,7 @@ def test_deterministic(rad):
 def test_direct_mode_many_tiles(rad, oracle_mod):
     """Grid large enough (>= 8 CTAs per SM) for the no-split path; sampled + lattice."""
     wl = workloads.make("cfg2", n=300, n_omega=40, n_th=200, seed=21)
-    rad.rad_set_kernel(1)                              # the direct-phasor kernel (auto would pick the separable one)
-    try:
-        cube = run_single(rad, wl, CL, 0.0)
-    finally:
-        rad.rad_set_kernel(0)
+    cube = run_single(rad, wl, CL, 0.0, kernel=1)      # the direct-phasor kernel (auto would pick the separable one)
     idx, ref = sampled_reference(oracle_mod, wl, cube, 3000, (5, 9, 9), CL, 0.0)
     assert_parity(cube, ref, idx, label="direct")
 
@@ -265,37 +262,32 @@ def test_angular_sum(rad):
 
 # ------------------------------------------------------------------ full-size configs, sampled
 @pytest.fixture(params=[0, 1, 2], ids=["auto", "direct", "separable"])
-def each_kernel(request, rad):
+def each_kernel(request):
     """The full-size configs run through the kernel the library picks (what bench.py times) and through
-    each of the two kernels forced (include/rad.h rad_set_kernel)."""
-    rad.rad_set_kernel(request.param)
-    yield rad
-    rad.rad_set_kernel(0)
+    each of the two kernels forced (include/rad.h rad_options.kernel)."""
+    return request.param
 
 
-def test_cfg2_full_size_sampled(each_kernel, oracle_mod):
+def test_cfg2_full_size_sampled(rad, each_kernel, oracle_mod):
     """BASELINE.json configs[1] at full size, in the launch configuration bench.py times."""
-    rad = each_kernel
     wl = workloads.make("cfg2")
-    cube = run_single(rad, wl, CL, 0.0)
+    cube = run_single(rad, wl, CL, 0.0, each_kernel)
     idx, ref = sampled_reference(oracle_mod, wl, cube, 3000, (8, 6, 6), CL, 0.0)
     assert_parity(cube, ref, idx, label="cfg2 full")
 
 
-def test_cfg3_full_size_sampled(each_kernel, oracle_mod):
+def test_cfg3_full_size_sampled(rad, each_kernel, oracle_mod):
     """BASELINE.json configs[2]: spin-1/2, N = 2e5, |phase| up to ~1e6 rad; 512 x 64 x 64 grid."""
-    rad = each_kernel
     wl = workloads.make("cfg3")
-    cube = run_single(rad, wl, SH, wl.hbarc_over_E)
+    cube = run_single(rad, wl, SH, wl.hbarc_over_E, each_kernel)
     idx, ref = sampled_reference(oracle_mod, wl, cube, 160, (4, 3, 3), SH, wl.hbarc_over_E)
     assert_parity(cube, ref, idx, label="cfg3 full")
 
 
-def test_cfg4_reduced_ensemble_sampled(each_kernel, oracle_mod):
+def test_cfg4_reduced_ensemble_sampled(rad, each_kernel, oracle_mod):
     """configs[3] shape (128 x 16 x 16 grid, batched trajectories) with 48 x 20000 samples."""
-    rad = each_kernel
     we = workloads.make("cfg4", count=48, n=20000)
-    cube = rad.rad_ensemble_sum(dev_dict(we.batch), we.n, *dev_grid(we)).cpu().numpy()
+    cube = rad.rad_ensemble_sum(dev_dict(we.batch), we.n, *dev_grid(we), kernel=each_kernel).cpu().numpy()
     idx = workloads.sample_points(we, 100, (4, 3, 3))
     idx = np.unique(np.concatenate([idx, [int(np.argmax(cube))]]))
     w, nx, ny = workloads.points_of(we, idx)
@@ -304,11 +296,10 @@ def test_cfg4_reduced_ensemble_sampled(each_kernel, oracle_mod):
 
 
 @pytest.mark.parametrize("model", [S0, SH])
-def test_cfg5_reduced_sampled(each_kernel, oracle_mod, model):
+def test_cfg5_reduced_sampled(rad, each_kernel, oracle_mod, model):
     """configs[4] (axial well, both spin variants) at N = 2e5 on the full 1024 x 64 x 64 grid."""
-    rad = each_kernel
     wl = workloads.make("cfg5", n=200000, model=model)
-    cube = run_single(rad, wl, model, wl.hbarc_over_E)
+    cube = run_single(rad, wl, model, wl.hbarc_over_E, each_kernel)
     idx, ref = sampled_reference(oracle_mod, wl, cube, 120, (4, 3, 3), model, wl.hbarc_over_E)
     assert_parity(cube, ref, idx, label=f"cfg5 model {model}")
 
@@ -357,11 +348,23 @@ def test_shards_run_sequentially_equal_unsharded(rad, oracle_mod):
 
 
 # ------------------------------------------------------------------ separable-phasor kernel (N2), forced
+class _Forced:
+    """The binding with one kernel forced on every compute call (rad_options.kernel is per call)."""
+
+    def __init__(self, rad, kernel):
+        self._rad, self._kernel = rad, kernel
+
+    def __getattr__(self, name):
+        fn = getattr(self._rad, name)
+        if name in ("rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_sections_sum", "rad_eval_host",
+                    "rad_ensemble_sum_host", "rad_angular_spectrum"):
+            return lambda *a, **k: fn(*a, **{**k, "kernel": self._kernel})
+        return fn
+
+
 @pytest.fixture
 def sep_kernel(rad):
-    rad.rad_set_kernel(2)
-    yield rad
-    rad.rad_set_kernel(0)
+    return _Forced(rad, 2)
 
 
 @pytest.mark.parametrize("model", [CL, S0, SH])
@@ -458,28 +461,27 @@ def test_sep_straight_line_domain_and_workspace(sep_kernel, oracle_mod):
 
 
 def test_plan_kernel_choice(rad):
-    """rad_plan_kernel: separable where the grid fills its tiles (BASELINE configs 2-5), direct on
-    small angle grids (config 1); rad_set_kernel overrides and is restored."""
+    """rad_plan_kernel: separable where the grid fills its tiles (BASELINE configs 2-5), direct on small angle
+    grids with long trajectories, the fused single-launch kernel on small problems (config 1); the per-call
+    option overrides; a bad option is rejected by the call itself."""
     assert rad.rad_plan_kernel(256, 32, 32, CL) == 2 and rad.rad_plan_kernel(512, 64, 64, SH) == 2
     assert rad.rad_plan_kernel(128, 16, 16, CL) == 2 and rad.rad_plan_kernel(1024, 64, 64, S0) == 2
-    assert rad.rad_plan_kernel(64, 8, 8, CL) == 1 and rad.rad_plan_kernel(5, 3, 3, SH) == 1
-    rad.rad_set_kernel(1)
-    assert rad.rad_plan_kernel(256, 32, 32, CL) == 1
-    rad.rad_set_kernel(2)
-    assert rad.rad_plan_kernel(5, 3, 3, SH) == 2
-    rad.rad_set_kernel(0)
-    with pytest.raises(rad.RadError):
-        rad.rad_set_kernel(7)
+    assert rad.rad_plan_kernel(64, 8, 8, CL) == 1 and rad.rad_plan_kernel(5, 3, 3, SH) == 1       # n_max = 2^20
+    assert rad.rad_plan_kernel(64, 8, 8, CL, n_max=4000) == 3 and rad.rad_plan_kernel(5, 3, 3, SH, n_max=900) == 3
+    assert rad.rad_plan_kernel(64, 8, 8, CL, n_max=4000, count=2) == 1
+    assert rad.rad_plan_kernel(256, 32, 32, CL, kernel=1) == 1
+    assert rad.rad_plan_kernel(5, 3, 3, SH, kernel=2) == 2
+    wl = workloads.make("cfg1", n=100, n_omega=4, n_th=2)
+    with pytest.raises(rad.RadError) as e:
+        rad.rad_classical(dev_dict(wl.traj), *dev_grid(wl), kernel=7)
+    assert e.value.code == -1
 
 
 def test_sep_matches_direct_kernel(rad, oracle_mod):
     """Both kernels on the same input agree far inside the tolerance (they share only the packed records)."""
     wl = workloads.make("cfg3", n=5000, n_omega=32, n_th=32)
-    rad.rad_set_kernel(1)
-    a = run_single(rad, wl, SH, wl.hbarc_over_E)
-    rad.rad_set_kernel(2)
-    b = run_single(rad, wl, SH, wl.hbarc_over_E)
-    rad.rad_set_kernel(0)
+    a = run_single(rad, wl, SH, wl.hbarc_over_E, kernel=1)
+    b = run_single(rad, wl, SH, wl.hbarc_over_E, kernel=2)
     tol = np.maximum(RTOL * np.abs(a), FLOOR * a.max())
     assert np.max(np.abs(a - b) / tol) <= 1.0
 
@@ -500,22 +502,19 @@ def test_sections_sum(rad, oracle_mod, kernel):
     for s in range(4):
         for k in tr:
             batch[k][s, :nvec[s]] = tr[k][start[s]:start[s + 1] + 1]
-    # the shared boundary sample belongs to both neighbours: give it each section's own gamma, as a caller would
+    # the shared boundary sample is ONE array entry read by both neighbours (include/rad.h, boundary-sample rule):
+    # it carries the NEW section's gamma here, and the oracle batch is cut from the same arrays
     trs = {k: v.copy() for k, v in tr.items()}
     w, nx, ny = oracle_mod.grid_points(wl.omega, wl.thx, wl.thy)
-    rad.rad_set_kernel(kernel)
-    try:
-        for model in (CL, SH):
-            ref = oracle_mod.ensemble_points(batch, nvec, w, nx, ny, model, lam if model else None)
-            cube = rad.rad_sections_sum(dev_dict(trs), start, *dev_grid(wl), model=model,
-                                        hbarc_over_E=lam if model else None).cpu().numpy()
-            assert_parity(cube, ref, label=f"sections kernel {kernel} model {model}")
-        half = rad.rad_sections_sum(dev_dict(trs), start[:3], *dev_grid(wl), model=SH, hbarc_over_E=lam[:2])
-        both = rad.rad_sections_sum(dev_dict(trs), start[2:], *dev_grid(wl), model=SH, hbarc_over_E=lam[2:],
-                                    accumulate=True, out=half).cpu().numpy()
-        assert_parity(both, ref, label=f"sections accumulate kernel {kernel}")
-    finally:
-        rad.rad_set_kernel(0)
+    for model in (CL, SH):
+        ref = oracle_mod.ensemble_points(batch, nvec, w, nx, ny, model, lam if model else None)
+        cube = rad.rad_sections_sum(dev_dict(trs), start, *dev_grid(wl), model=model,
+                                    hbarc_over_E=lam if model else None, kernel=kernel).cpu().numpy()
+        assert_parity(cube, ref, label=f"sections kernel {kernel} model {model}")
+    half = rad.rad_sections_sum(dev_dict(trs), start[:3], *dev_grid(wl), model=SH, hbarc_over_E=lam[:2], kernel=kernel)
+    both = rad.rad_sections_sum(dev_dict(trs), start[2:], *dev_grid(wl), model=SH, hbarc_over_E=lam[2:],
+                                accumulate=True, out=half, kernel=kernel).cpu().numpy()
+    assert_parity(both, ref, label=f"sections accumulate kernel {kernel}")
     with pytest.raises(rad.RadError):
         rad.rad_sections_sum(dev_dict(trs), [0, 10, 10], *dev_grid(wl))
     with pytest.raises(rad.RadError):
@@ -538,11 +537,7 @@ def test_million_samples_on_a_small_grid(rad, oracle_mod, kernel):
     """configs[4]'s trajectory length (N = 1e6, phases to 3.8e6 rad) on a grid small enough that the time
     axis is split across the whole GPU (7813 chunks), both kernels, spin-1/2."""
     wl = workloads.make("cfg5", n=1000000, n_omega=16, n_th=16)
-    rad.rad_set_kernel(kernel)
-    try:
-        cube = run_single(rad, wl, SH, wl.hbarc_over_E)
-    finally:
-        rad.rad_set_kernel(0)
+    cube = run_single(rad, wl, SH, wl.hbarc_over_E, kernel=kernel)
     idx, ref = sampled_reference(oracle_mod, wl, cube, 40, (3, 3, 3), SH, wl.hbarc_over_E)
     assert_parity(cube, ref, idx, label=f"N=1e6 kernel {kernel}")
 
@@ -571,8 +566,8 @@ def test_cfg4_full_size_sampled(rad, oracle_mod):
 
 
 def test_angular_spectrum_in_slabs(rad, oracle_mod):
-    """rad_angular_spectrum: dI/dw slab by slab (3 slabs of <= 16 omegas here) without the 460 MB cube of the
-    whole grid; equals cube + rad_angular_sum, and the oracle's sum on a small grid."""
+    """rad_angular_spectrum without the 460 MB cube of the whole grid (the sums come out of the main kernel's
+    epilogue); equals cube + rad_angular_sum, and the oracle's sum on a small grid (cube path inside the workspace)."""
     import torch
     wl = workloads.make("cfg2", n=120, n_omega=40, n_th=1200, seed=19)
     g = dev_grid(wl)
@@ -581,6 +576,7 @@ def test_angular_spectrum_in_slabs(rad, oracle_mod):
     b = {k: v[None, :].contiguous() for k, v in dev_dict(wl.traj).items()}
     n = np.array([120], dtype=np.int64)
     assert rad.load_library().rad_angular_spectrum_workspace_bytes(1, 120, 40, 1200, 1200) < 1200 * 1200 * 8 * 20
+    assert rad.rad_plan_describe(1, 120, 40, 1200, 1200)["mode"] == 0      # one CTA per tile: sums in the epilogue
     got = rad.rad_angular_spectrum(b, n, *g, d_om, cut).cpu().numpy()
     cube = rad.rad_classical(dev_dict(wl.traj), *g)
     want = rad.rad_angular_sum(cube, *g, d_om, cut).cpu().numpy()
@@ -602,24 +598,224 @@ def test_single_trajectory_call_is_graph_capturable(rad):
     """With a caller workspace a single-trajectory call only enqueues kernels (no host sync, no allocation, no
     host copy), so it can be captured in a CUDA graph and replayed; replays reproduce the eager bits."""
     import torch
-    for shape, kernel in ((dict(n=900, n_omega=16, n_th=6), 1), (dict(n=900, n_omega=32, n_th=16), 2)):
+    for shape, kernel in ((dict(n=900, n_omega=16, n_th=6), 1), (dict(n=900, n_omega=32, n_th=16), 2),
+                          (dict(n=900, n_omega=16, n_th=6), 3)):
         wl = workloads.make("cfg2", seed=4, **shape)
         tr, g = dev_dict(wl.traj), dev_grid(wl)
-        assert rad.rad_plan_kernel(len(wl.omega), len(wl.thx), len(wl.thy), SH) == kernel
         lam = 0.4 / wl.omega.max()
         ws = torch.empty(rad.rad_workspace_bytes(1, 900, len(wl.omega), len(wl.thx), len(wl.thy)),
                          dtype=torch.uint8, device="cuda")
         out = torch.zeros((len(wl.omega), len(wl.thy), len(wl.thx)), dtype=torch.float64, device="cuda")
-        eager = rad.rad_semiclassical(tr, *g, 1, lam, workspace=ws).clone()        # also warms up the kernels
+        eager = rad.rad_semiclassical(tr, *g, 1, lam, workspace=ws, kernel=kernel).clone()   # also warms up the kernels
         graph = torch.cuda.CUDAGraph()
         side = torch.cuda.Stream()
         side.wait_stream(torch.cuda.current_stream())
         with torch.cuda.stream(side):
             with torch.cuda.graph(graph, stream=side):
-                rad.rad_semiclassical(tr, *g, 1, lam, out=out, workspace=ws)
+                rad.rad_semiclassical(tr, *g, 1, lam, out=out, workspace=ws, kernel=kernel)
         torch.cuda.current_stream().wait_stream(side)
         for _ in range(3):
             out.zero_()
             graph.replay()
             torch.cuda.synchronize()
             assert torch.equal(out, eager)
+
+
+# ------------------------------------------------------------------ fused single-launch kernel (row a6, small problems)
+def test_fused_kernel_is_what_cfg1_runs(rad, oracle_mod):
+    """BASELINE configs[0] through the library's own choice: ONE launch (pack, time split over all SMs, grid-wide
+    ordered reduction, epilogue), full grid against the oracle, deterministic, accumulate adds."""
+    wl = workloads.make("cfg1")
+    plan = rad.rad_plan_describe(1, 4000, 64, 8, 8)
+    assert plan["kernel"] == 3 and plan["launches"] == 1
+    tr, g = dev_dict(wl.traj), dev_grid(wl)
+    n0 = rad.rad_launch_count()
+    cube = rad.rad_classical(tr, *g)
+    assert rad.rad_launch_count() - n0 == 1
+    ref = oracle_mod.grid(wl.traj, wl.omega, wl.thx, wl.thy)
+    assert_parity(cube.cpu().numpy(), ref, label="cfg1 fused")
+    assert np.array_equal(cube.cpu().numpy(), rad.rad_classical(tr, *g).cpu().numpy())
+    direct = rad.rad_classical(tr, *g, kernel=1).cpu().numpy()          # the three-launch path, same arithmetic per sample
+    tol = np.maximum(RTOL * np.abs(direct), FLOOR * direct.max())
+    assert np.max(np.abs(direct - cube.cpu().numpy()) / tol) <= 1e-3
+
+
+@pytest.mark.parametrize("model", [CL, S0, SH])
+@pytest.mark.parametrize("shape", [dict(n=2, n_omega=1, n_th=1), dict(n=63, n_omega=3, n_th=2), dict(n=129, n_omega=9, n_th=3),
+                                   dict(n=1037, n_omega=13, n_th=5), dict(n=5000, n_omega=17, n_th=17)])
+def test_fused_kernel_ragged_shapes_all_models(rad, oracle_mod, model, shape):
+    """Forced fused kernel: n below / not a multiple of its 64-sample rounds, omega count not a multiple of 8,
+    thread count not a multiple of 64, more time slices than samples allow."""
+    wl = workloads.make("cfg2", seed=13, **shape)
+    lam = 0.6 / wl.omega.max()
+    cube = run_single(rad, wl, model, lam, kernel=3)
+    ref = oracle_mod.grid(wl.traj, wl.omega, wl.thx, wl.thy, model, lam)
+    assert_parity(cube, ref, label=f"fused ragged {shape} model {model}")
+
+
+def test_fused_kernel_edges(rad, oracle_mod):
+    """Straight line -> exactly 0; u >= 1 -> NaN only there; non-uniform t and varying gamma; long trajectory on a tiny
+    grid (forced: auto would take the TMA-pipelined path); refused where it does not apply."""
+    wl = workloads.make("cfg2", n=500, n_omega=8, n_th=4)
+    for k in ("ax", "ay", "az"):
+        wl.traj[k] = np.zeros(500)
+    for model in (CL, S0, SH):
+        assert np.all(run_single(rad, wl, model, 1e-16, kernel=3) == 0.0)
+    wl = workloads.make("cfg1", n=600, n_omega=8, n_th=2)
+    lam = 1.0000001 / wl.omega[5]
+    cube = run_single(rad, wl, SH, lam, kernel=3)
+    assert np.all(np.isnan(cube[5:])) and np.all(np.isfinite(cube[:5]))
+    assert_parity(cube[:5], oracle_mod.grid(wl.traj, wl.omega[:5], wl.thx, wl.thy, SH, lam), label="fused domain")
+    wl = workloads.make("cfg2", n=900, n_omega=10, n_th=4, seed=8)
+    rng = np.random.Generator(np.random.PCG64(3))
+    t = np.sort(rng.uniform(0, wl.traj["t"][-1], 900))
+    tr = {k: np.interp(t, wl.traj["t"], v) for k, v in wl.traj.items()}
+    tr["t"] = t
+    tr["gamma"] = wl.traj["gamma"] * (1 - 1e-3 * np.linspace(0, 1, 900))
+    wl.traj = tr
+    lam = 0.5 / wl.omega.max()
+    assert_parity(run_single(rad, wl, SH, lam, kernel=3), oracle_mod.grid(tr, wl.omega, wl.thx, wl.thy, SH, lam),
+                  label="fused nonuniform")
+    wl = workloads.make("cfg5", n=100000, n_omega=8, n_th=4)
+    cube = run_single(rad, wl, SH, wl.hbarc_over_E, kernel=3)
+    assert_parity(cube, oracle_mod.grid(wl.traj, wl.omega, wl.thx, wl.thy, SH, wl.hbarc_over_E), label="fused N=1e5")
+    big = workloads.make("cfg2", n=200, n_omega=64, n_th=128)
+    with pytest.raises(rad.RadError) as e:
+        run_single(rad, big, CL, 0.0, kernel=3)                         # 2048 tiles of 64 threads: more CTAs than fit at once
+    assert e.value.code == -1
+    we = workloads.make("cfg4", count=2, n=300, n_omega=4, n_th=2)
+    with pytest.raises(rad.RadError):
+        rad.rad_ensemble_sum(dev_dict(we.batch), we.n, *dev_grid(we), kernel=3)
+
+
+# ------------------------------------------------------------------ two-part plan: separable interior + direct L-shaped rest
+@pytest.mark.parametrize("model", [CL, SH])
+def test_papers_typical_grid_in_two_parts(rad, oracle_mod, model):
+    """PAPER.md:149's typical grid with multiple scattering, N_x = N_y = 50, N_w = 100, N = 3000: the
+    library's own plan (separable kernel on 48 x 48 angles, direct kernel on the other 196), full grid against the
+    oracle; the output of both parts lands in the one cube with the right strides."""
+    wl = workloads.make("paper_typical", model=model)
+    plan = rad.rad_plan_describe(1, len(wl.traj["t"]), 100, 50, 50, model)
+    assert (plan["parts"], plan["interior_x"], plan["interior_y"]) == (2, 48, 48)
+    lam = wl.hbarc_over_E
+    cube = run_single(rad, wl, model, lam)
+    assert cube.shape == (100, 50, 50)
+    ref = oracle_mod.grid(wl.traj, wl.omega, wl.thx, wl.thy, model, lam)
+    assert_parity(cube, ref, label=f"paper typical model {model}")
+
+
+def test_two_parts_rectangular_rest_on_one_axis_and_ensemble(rad, oracle_mod):
+    """Only one axis leaves a rest (50 x 32: columns 48, 49), n_thx != n_thy, an ensemble with accumulate; against the
+    oracle on a sample of points that covers interior, rest and the corners."""
+    we = workloads.make("cfg4", count=3, n=2500, n_omega=40, n_th=50, seed0=77)
+    we.thy = we.thy[:32].copy()
+    plan = rad.rad_plan_describe(3, 2500, 40, 50, 32)
+    assert (plan["parts"], plan["interior_x"], plan["interior_y"]) == (2, 48, 32)
+    b, g = dev_dict(we.batch), dev_grid(we)
+    first = rad.rad_ensemble_sum({k: v[:1].contiguous() for k, v in b.items()}, we.n[:1], *g)
+    cube = rad.rad_ensemble_sum({k: v[1:].contiguous() for k, v in b.items()}, we.n[1:], *g, accumulate=True,
+                                out=first).cpu().numpy()
+    assert cube.shape == (40, 32, 50)
+    rng = np.random.Generator(np.random.PCG64(5))
+    iw, iy, ix = rng.integers(0, 40, 600), rng.integers(0, 32, 600), rng.integers(0, 50, 600)
+    ix[:200] = rng.integers(48, 50, 200)                                # the rest columns
+    idx = np.unique(np.concatenate([(iw * 32 + iy) * 50 + ix, [0, 49, 31 * 50, 40 * 32 * 50 - 1, int(np.argmax(cube))]]))
+    W_, Y_, X_ = np.unravel_index(idx, cube.shape)
+    ref = oracle_mod.ensemble_points(we.batch, we.n, we.omega[W_], we.thx[X_], we.thy[Y_])
+    assert_parity(cube, ref, idx, label="two parts ensemble")
+
+
+# ------------------------------------------------------------------ angular spectrum from the epilogue (NEXT row N1)
+@pytest.mark.parametrize("kernel", [1, 2])
+@pytest.mark.parametrize("model", [CL, SH])
+def test_angular_spectrum_fused_against_the_oracle(rad, oracle_mod, kernel, model):
+    """dI/dw = dOmega * sum over the angles inside the collimator of the ORACLE's cube, with a real solid-angle element
+    and an active theta cut whose mask is computed here from the grid arrays; grid big enough (400 x 400 angles x 32
+    omegas) that the sums come out of the main kernel's epilogue, through both kernels."""
+    wl = workloads.make("cfg3" if model == SH else "cfg2", n=90, n_omega=32, n_th=400, seed=29)
+    lam = wl.hbarc_over_E if model == SH else 0.0
+    plan = rad.rad_plan_describe(1, 90, 32, 400, 400, model, kernel)
+    assert plan["mode"] == 0 and plan["kernel"] == kernel
+    d_om = (wl.thx[1] - wl.thx[0]) * (wl.thy[1] - wl.thy[0])
+    cut = 0.6 * wl.thx.max()
+    b = {k: v[None, :].contiguous() for k, v in dev_dict(wl.traj).items()}
+    got = rad.rad_angular_spectrum(b, np.array([90]), *dev_grid(wl), d_om, cut, model=model,
+                                   hbarc_over_E=lam if model else None, kernel=kernel).cpu().numpy()
+    X, Y = np.meshgrid(wl.thx, wl.thy)
+    mask = X * X + Y * Y <= cut * cut
+    assert 0.2 < mask.mean() < 0.4                                       # the cut is active
+    ref_cube = oracle_mod.grid(wl.traj, wl.omega, wl.thx, wl.thy, model, lam)
+    ref = (ref_cube * mask).sum((1, 2)) * d_om
+    # every term is >= 0, so the sum of N terms each within 1e-9 relative / 1e-12 S_max absolute stays within that
+    tol = np.maximum(RTOL * np.abs(ref), FLOOR * ref_cube.max() * mask.sum() * d_om)
+    assert np.max(np.abs(got - ref) / tol) <= 1.0
+    unmasked = rad.rad_angular_spectrum(b, np.array([90]), *dev_grid(wl), d_om, 0.0, model=model,
+                                        hbarc_over_E=lam if model else None, kernel=kernel).cpu().numpy()
+    ref_all = ref_cube.sum((1, 2)) * d_om
+    assert np.max(np.abs(unmasked - ref_all) / np.maximum(RTOL * ref_all, FLOOR * ref_cube.max() * mask.size * d_om)) <= 1.0
+    assert np.all(unmasked >= got)
+
+
+def test_angular_spectrum_three_thousand_squared_sampled_per_omega(rad, oracle_mod):
+    """"more than 3000 points in both spatial dimension ... approach the limit" of memory.  3000 x 3000
+    angles x 24 omegas = 2.2e8 integrals: the 1.7 GB cube is never written; two omegas are checked against the oracle's
+    sum over all 9e6 angles (collimator cut active), the rest against the ensemble identity sum_p = p-fold."""
+    wl = workloads.make("cfg2", n=48, n_omega=24, n_th=3000, seed=37)
+    d_om = (wl.thx[1] - wl.thx[0]) * (wl.thy[1] - wl.thy[0])
+    cut = 0.8 * wl.thx.max()
+    need = rad.load_library().rad_angular_spectrum_workspace_bytes(1, 48, 24, 3000, 3000)
+    assert need < 24 * 3000 * 3000 * 8 / 4                              # far below the cube
+    b = {k: v[None, :].contiguous() for k, v in dev_dict(wl.traj).items()}
+    got = rad.rad_angular_spectrum(b, np.array([48]), *dev_grid(wl), d_om, cut).cpu().numpy()
+    X, Y = np.meshgrid(wl.thx, wl.thy)
+    mask = (X * X + Y * Y <= cut * cut).ravel()
+    for iw in (3, 20):
+        vals = oracle_mod.points(wl.traj, np.full(mask.sum(), wl.omega[iw]), X.ravel()[mask], Y.ravel()[mask])
+        ref = vals.sum() * d_om
+        assert abs(got[iw] - ref) <= max(RTOL * ref, FLOOR * vals.max() * mask.sum() * d_om)
+    twice = rad.rad_angular_spectrum({k: v.repeat(2, 1) for k, v in b.items()}, np.array([48, 48]), *dev_grid(wl), d_om,
+                                     cut).cpu().numpy()
+    np.testing.assert_allclose(twice, 2 * got, rtol=1e-13)
+
+
+def test_angular_spectrum_small_grid_with_cut(rad, oracle_mod):
+    """Grids too small to give every SM its tiles take the cube path inside the workspace (the cube is then < 40 MB);
+    same contract: real solid-angle element, active cut, against the oracle; workspace exactly as the library asks."""
+    import torch
+    ws = workloads.make("cfg3", n=800, n_omega=9, n_th=21, seed=23)
+    assert rad.rad_plan_describe(1, 800, 9, 21, 21, SH)["mode"] != 0
+    d_om = (ws.thx[1] - ws.thx[0]) * (ws.thy[1] - ws.thy[0])
+    cut = 0.7 * ws.thx.max()
+    b = {k: v[None, :].contiguous() for k, v in dev_dict(ws.traj).items()}
+    need = rad.load_library().rad_angular_spectrum_workspace_bytes(1, 800, 9, 21, 21)
+    wsp = torch.empty(need, dtype=torch.uint8, device="cuda")
+    got = rad.rad_angular_spectrum(b, np.array([800]), *dev_grid(ws), d_om, cut, model=SH, hbarc_over_E=ws.hbarc_over_E,
+                                   workspace=wsp).cpu().numpy()
+    X, Y = np.meshgrid(ws.thx, ws.thy)
+    mask = X * X + Y * Y <= cut * cut
+    assert 0.2 < mask.mean() < 0.6
+    cube = oracle_mod.grid(ws.traj, ws.omega, ws.thx, ws.thy, SH, ws.hbarc_over_E)
+    ref = (cube * mask).sum((1, 2)) * d_om
+    assert np.max(np.abs(got - ref) / np.maximum(RTOL * ref, FLOOR * cube.max() * mask.sum() * d_om)) <= 1.0
+
+
+def test_number_spectrum(rad):
+    import torch
+    spec = torch.tensor([1.0, 4.0, 9.0], dtype=torch.float64, device="cuda")
+    om = torch.tensor([2.0, 4.0, 0.5], dtype=torch.float64, device="cuda")
+    got = rad.rad_number_spectrum(spec, om, 0.25).cpu().numpy()
+    assert np.array_equal(got, np.array([1.0 / 0.5, 4.0 / 1.0, 9.0 / 0.125]))
+    with pytest.raises(rad.RadError):
+        rad.rad_number_spectrum(spec, om, 0.0)
+
+
+def test_profile_object_times_one_call(rad):
+    """rad_options.profile: per-call events; two profiles used by two calls do not disturb each other."""
+    wl = workloads.make("cfg2", n=3000, n_omega=32, n_th=16)
+    tr, g = dev_dict(wl.traj), dev_grid(wl)
+    p1, p2 = rad.RadProfile(), rad.RadProfile()
+    rad.rad_classical(tr, *g, profile=p1, kernel=2)
+    rad.rad_classical(tr, *g, profile=p2, kernel=3 if rad.rad_plan_kernel(32, 16, 16, CL, kernel=0, n_max=3000) == 3 else 1)
+    a, b_ = p1.read(), p2.read()
+    assert a[1] > 0 and b_[1] > 0 and a[0] >= 0 and a[2] > 0
+    p1.close(); p2.close()

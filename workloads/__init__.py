@@ -286,7 +286,28 @@ def config5(n: int = 1000000, n_omega: int = 1024, n_th: int = 64, seed: int = 5
         meta={"gamma": gamma, "E_eV": E, "seed": seed})
 
 
-CONFIGS = {"cfg1": config1, "cfg2": config2, "cfg3": config3, "cfg4": config4, "cfg5": config5}
+def paper_typical(n: int = 3000, n_omega: int = 100, n_th: int = 50, seed: int = 6, model: int = CLASSICAL) -> Workload:
+    """The grid the paper calls typical "when multiple scattering is included" (N_x = N_y = 50,
+    N_omega = 100) over its benchmark trajectory length (3000 time points): the config-2 recipe
+    (5 GeV e+, harmonic well, scattering kicks), 50 uniform angles in +-3/gamma, 100 log-spaced omegas.  Not a
+    BASELINE.json config: a shape whose angle counts are not multiples of the kernels' tiles."""
+    E = 5e9
+    gamma = E / ME_EV
+    w_p = 2.0 * math.pi / 7e-6
+    dt = 7e-9
+    b = _harmonic_ms([seed], n, dt, gamma, w_p, 0.96e-10, 2e-7)
+    tr = {k: v[0] for k, v in b.items()}
+    w_c = 2.0 * gamma ** 2 * w_p
+    return Workload(
+        name=f"paper_typical_50x50x100_model{model}", model=model,
+        omega=_logspace(0.05 * w_c, 10.0 * w_c, n_omega),
+        thx=_uniform_sym(3.0 / gamma, n_th), thy=_uniform_sym(3.0 / gamma, n_th),
+        traj=tr, hbarc_over_E=0.0 if model == CLASSICAL else HBARC_EV_M / E,
+        meta={"gamma": gamma, "E_eV": E, "seed": seed})
+
+
+CONFIGS = {"cfg1": config1, "cfg2": config2, "cfg3": config3, "cfg4": config4, "cfg5": config5,
+           "paper_typical": paper_typical}
 
 
 def make(name: str, **overrides) -> Workload:
