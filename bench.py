@@ -1,22 +1,29 @@
 #!/usr/bin/env python
 """bench.py -- throughput of the radiation-integral hot path on B200 (one JSON line on stdout).
 
-    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg2|cfg1|cfg3|cfg4|cfg5]
-    python bench.py --impl reference ...     # the CPU oracle on the host cores, same metric
+    python bench.py [--gpus N] [--steps K] [--warmup W] [--workload cfg5|cfg1|cfg2|cfg3|cfg4|paper_typical]
+    python bench.py --impl reference ...     # the CPU oracle on the host cores, same metric and workload
 
-A "step" is one pass of the whole hot path -- pack, main kernel, ordered reduction (SURVEY.md
-section 8(a) rows a0-a7) -- over one synthetic batch: by default BASELINE.json configs[1]
-(classical, 5 GeV planar-channeling positron, N = 14287 samples, 256 x 32 x 32 grid).
-metric = FP64 radiation-integral evals/s (grid points x time steps), BASELINE.json `metric`.
+A "step" is one pass of the whole hot path -- pack, main kernel(s), ordered reduction (SURVEY.md section 8(a)
+rows a0-a7) -- over one synthetic batch.  Default workload: BASELINE.json configs[4] with the spin-1/2 model
+(50 GeV axial channeling, N = 1e6 samples, 1024 x 64 x 64 grid: the largest single-GPU configuration, which
+BASELINE.json's `metric` -- it names no config -- is therefore quoted on).  metric = FP64 radiation-integral
+evals/s (grid points x time steps), BASELINE.json `metric`.
 
-  value      device-resident inputs, CUDA events on the launching stream, L2 flushed between steps
-  e2e        same step through the C-ABI host-buffer call (pinned host memory, H2D + D2H inside)
-  roofline   main kernel only: algorithmic flops (flops per eval x evals per launch)
-             / its own event-timed duration, against the FP64 FMA peak measured in this run
-  cpu_baseline  the CPU oracle (oracle/, double build of the same source) on a bounded sample
+  value        device-resident inputs, CUDA events on the launching stream, L2 flushed between steps
+  e2e          same step through the C-ABI host-buffer call (pinned host memory, H2D + D2H inside)
+  roofline     main kernel(s) only: algorithmic flops (flops per eval x evals per launch) / their own
+               event-timed duration (rad_options.profile), against the FP64 FMA peak measured in this run
+  per_config   the other target configurations (cfg2 classical, cfg3 spin-1/2, cfg4 ensemble, cfg5 spin-0), config 1
+               and the paper's typical 50 x 50 x 100 grid, each with its own value / roofline / clocks, and the
+               direct (one phasor per eval) kernel beside the default one where the time budget allows
+  cpu_baseline the CPU oracle (oracle/, double build of the same source) on a bounded sample
 
-N > 1 (torchrun, one rank per GPU): each rank evaluates its own trajectory of the workload
-(independent problems, no data-path collective; weak scaling); value = all ranks' evals / max time.
+N > 1 (torchrun, one rank per GPU): the SAME job sharded (paper_1910_10391_b200/sharding.py) --
+the headline grid cut into omega slabs (no exchange in the computation; the optional gather of the cube is outside
+the metric), and in per_config the cfg4 ensemble dealt out by trajectories with ONE exchange (all-gather of the
+partial cubes + ordered sum) inside the timed region.  Strong scaling: value = the whole job's evals / max-over-ranks
+device time.
 """
 from __future__ import annotations
 
@@ -35,53 +42,51 @@ sys.path.insert(0, str(ROOT))
 
 METRIC = "fp64_radiation_integral_evals_per_s"
 UNIT = "evals/s"
-# algorithmic FP64 flops per eval, enumerated there operation by operation.
-# Direct kernel: phase 2, exact range reduction 1 (+ one FRND beside the FP64 pipe), quarter-angle
-# polynomials 21, two doublings 7, complex accumulation 8 [+4 for spin-1/2's J], integrand geometry
-# 34 [37] per 8 omegas -> 43.25 [47.6] flops, 24.6 [26.9] FP64 instructions (SURVEY.md 8(d) estimated 52-60).
-# The separable-phasor kernel needs far fewer: per eval one complex multiply (6) and
-# the accumulation (8 [12]), plus per 16 [8] evals one T and one [half a] Y phasor and one [half an]
-# integrand entry (36 + 35 + 28 [31] flops) -> 20.19 [26.63] flops, 11.75 [15.19] FP64 instructions.
-# Both are checked against ncu's 2*DFMA + DMUL + DADD count (profiles/).
-KERNELS = {1: "rad_main_kernel (direct phasor)", 2: "rad_sep_kernel (separable phasor)"}
-FLOPS_PER_EVAL = {1: {0: 43.25, 1: 43.25, 2: 47.6}, 2: {0: 20.19, 1: 20.19, 2: 26.63}}
-FP64_INSTR_PER_EVAL = {1: {0: 24.6, 1: 24.6, 2: 26.9}, 2: {0: 11.75, 1: 11.75, 2: 15.19}}
-# dram__bytes_read.sum + dram__bytes_write.sum of ONE launch of the main kernel, from the ncu --set full
-# captures under profiles/ (r01_*_ncu_full.txt); bench.py cannot run ncu itself, other workloads report null.
-NCU_TRAFFIC_BYTES = {("cfg2", 2): 1.256704e6 + 75.79136e6, ("cfg2", 1): 1.2224e6 + 8.14976e6,
-                     ("cfg3", 2): 16.3904e6 + 10496.0, ("cfg3", 1): 16.240128e6 + 6144.0}
+# algorithmic FP64 flops per eval, enumerated there operation by operation and checked against
+# ncu's 2*DFMA + DMUL + DADD count (profiles/).  Direct kernel (also the fused single-launch kernel, which runs
+# the same per-sample body): phase 2, exact range reduction 1 (+ one FRND beside the FP64 pipe), quarter-angle
+# polynomials 21, two doublings 7, complex accumulation 8 [+4 for spin-1/2's J], integrand geometry 34 [37] per
+# 8 omegas -> 43.25 [47.6] flops, 24.6 [26.9] FP64 instructions (SURVEY.md 8(d) estimated 52-60).  Separable-phasor
+# kernel: per eval one complex multiply (6) and the accumulation (8 [12]), plus per 16 [8] evals one T and one
+# [half a] Y phasor and one [half an] integrand entry (36 + 35 + 28 [31] flops) -> 20.19 [26.63] flops, 11.75 [15.19]
+# FP64 instructions.
+KERNELS = {1: "rad_main_kernel (direct phasor)", 2: "rad_sep_kernel (separable phasor)",
+           3: "rad_fused_kernel (single launch: pack + direct phasor + grid-wide ordered reduction)"}
+FLOPS_PER_EVAL = {1: {0: 43.25, 1: 43.25, 2: 47.6}, 2: {0: 20.19, 1: 20.19, 2: 26.63}, 3: {0: 43.25, 1: 43.25, 2: 47.6}}
+FP64_INSTR_PER_EVAL = {1: {0: 24.6, 1: 24.6, 2: 26.9}, 2: {0: 11.75, 1: 11.75, 2: 15.19}, 3: {0: 24.6, 1: 24.6, 2: 26.9}}
 FP64_SPEC_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # 148 SM x 64 FMA lanes x 2 x 1.965 GHz
+MODELS = ["classical", "spin0", "spin1/2"]
+# dram__bytes_read.sum + dram__bytes_write.sum per main-kernel launch from the committed ncu --set full captures
+# (bench.py cannot run ncu itself): profiles/r02_ncu_traffic.json, written next to the captures it summarises.
+TRAFFIC_FILE = ROOT / "profiles" / "r02_ncu_traffic.json"
 
 
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=5)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", choices=["b200", "reference"], default="b200")
-    ap.add_argument("--workload", default="cfg2")
+    ap.add_argument("--workload", default="cfg5")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-per-config", action="store_true", help="headline workload only")
     ap.add_argument("--cfg4-count", type=int, default=1000)
-    ap.add_argument("--kernel", choices=["auto", "direct", "separable"], default="auto",
-                    help="main kernel of the timed steps (auto: the library's own choice by grid shape)")
+    ap.add_argument("--kernel", choices=["auto", "direct", "separable", "fused"], default="auto",
+                    help="main kernel of the timed steps (auto: the library's own choice by shape)")
     ap.add_argument("--spin", choices=["0", "1/2"], default="1/2",
                     help="semi-classical variant of cfg3 / cfg5 (BASELINE.json configs[4] asks for both)")
     return ap.parse_args()
 
 
-def make_workload(name: str, rank: int, cfg4_count: int, spin: str = "1/2"):
+def make_workload(name: str, cfg4_count: int = 1000, spin: str = "1/2"):
     import workloads
     model = workloads.SPIN0 if spin == "0" else workloads.SPIN_HALF
-    if name == "cfg2":
-        return workloads.make("cfg2", seed=2 + 1000 * rank)
-    if name == "cfg1":
-        return workloads.make("cfg1")
-    if name == "cfg3":
-        return workloads.make("cfg3", seed=3 + 1000 * rank, model=model)
+    if name in ("cfg1", "cfg2", "paper_typical"):
+        return workloads.make(name)
+    if name in ("cfg3", "cfg5"):
+        return workloads.make(name, model=model)
     if name == "cfg4":
-        return workloads.make("cfg4", count=cfg4_count, seed0=4000 + 100000 * rank)
-    if name == "cfg5":
-        return workloads.make("cfg5", seed=5 + 1000 * rank, model=model)
+        return workloads.make("cfg4", count=cfg4_count)
     raise SystemExit(f"unknown workload {name}")
 
 
@@ -162,10 +167,10 @@ def cpu_baseline(wl):
     samples = int(np.sum(wl.n)) if wl.batch is not None else len(wl.traj["t"])
     # size the sample for roughly 10-20 s of wall time on this box
     rate_guess = 2.0e7 * oracle.threads("f64")
-    npts = int(min(wl.n_points, max(256, 12.0 * rate_guess / samples)))
-    oracle_sample_rate(wl, min(npts, 512), "f64")                      # page in / warm up
+    npts = int(min(wl.n_points, max(64, 12.0 * rate_guess / samples)))
+    oracle_sample_rate(wl, min(npts, 64), "f64")                       # page in / warm up
     rate, got, secs = oracle_sample_rate(wl, npts, "f64")
-    npts_ld = max(64, npts // 16)
+    npts_ld = max(16, npts // 16)
     rate_ld, got_ld, secs_ld = oracle_sample_rate(wl, npts_ld, "ld")
     return {"value": rate, "unit": UNIT, "cores": oracle.threads("f64"), "kind": "oracle",
             "sample": (f"{got} seeded grid points x {samples} samples of {wl.name}, double build of "
@@ -182,11 +187,11 @@ def run_reference(args):
         return 0
     import oracle
     oracle.build_all()
-    wl = make_workload(args.workload, 0, min(args.cfg4_count, 8), args.spin)
+    wl = make_workload(args.workload, min(args.cfg4_count, 8), args.spin)
     samples = int(np.sum(wl.n)) if wl.batch is not None else len(wl.traj["t"])
     cores = oracle.threads("f64")
     budget_s = 90.0 / max(1, args.steps + args.warmup)
-    npts = int(min(wl.n_points, max(64, budget_s * 2.0e7 * cores / samples)))
+    npts = int(min(wl.n_points, max(16, budget_s * 2.0e7 * cores / samples)))
     for _ in range(args.warmup):
         oracle_sample_rate(wl, npts, "f64")
     total_t = 0.0
@@ -198,7 +203,7 @@ def run_reference(args):
     sample = f"{got} seeded grid points x {samples} samples of {wl.name} per step, double build, OpenMP"
     line = {"metric": METRIC, "value": value, "unit": UNIT, "impl": "reference", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total_t / args.steps,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic", "config": {"workload": wl.name, "sample_points_per_step": got},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -208,171 +213,272 @@ def run_reference(args):
 
 
 # ----------------------------------------------------------------------------- the B200 arm
-def run_b200(args):
-    import torch
-    import torch.distributed as dist
+class Bench:
+    def __init__(self, args):
+        import torch
+        import torch.distributed as dist
 
-    import paper_1910_10391_b200 as rad
+        import paper_1910_10391_b200 as rad
+        self.torch, self.dist, self.rad, self.args = torch, dist, rad, args
+        self.world = int(os.environ.get("WORLD_SIZE", "1"))
+        self.rank = int(os.environ.get("RANK", "0"))
+        self.local = int(os.environ.get("LOCAL_RANK", "0"))
+        if not torch.cuda.is_available():
+            raise SystemExit("bench.py needs a CUDA device: the CUDA path has no CPU fallback")
+        torch.cuda.set_device(self.local)
+        self.dev = torch.device("cuda", self.local)
+        if self.world > 1:
+            dist.init_process_group("nccl", device_id=self.dev)     # NCCL_DEBUG is left to the caller's environment
+        rad.build_library()
+        rad.load_library()
+        self.flush = torch.empty(256 << 20, dtype=torch.uint8, device=self.dev)      # > 126 MB L2
+        self.peak = rad.rad_measure_fp64_peak(300.0)                                 # FLOP/s, measured here
+        self.prof = rad.RadProfile()
+        try:
+            self.traffic = json.loads(TRAFFIC_FILE.read_text())
+        except Exception:
+            self.traffic = {}
 
-    world = int(os.environ.get("WORLD_SIZE", "1"))
-    rank = int(os.environ.get("RANK", "0"))
-    local = int(os.environ.get("LOCAL_RANK", "0"))
-    if not torch.cuda.is_available():
-        raise SystemExit("bench.py needs a CUDA device: the CUDA path has no CPU fallback")
-    torch.cuda.set_device(local)
-    dev = torch.device("cuda", local)
-    if world > 1:
-        dist.init_process_group("nccl", device_id=dev)
-    rad.build_library()
-    rad.load_library()
+    def barrier(self):
+        if self.world > 1:
+            self.dist.barrier()
+        self.torch.cuda.synchronize()
 
-    wl = make_workload(args.workload, rank, args.cfg4_count, args.spin)
-    model, lam = wl.model, wl.hbarc_over_E
-    grid = [torch.from_numpy(np.ascontiguousarray(a)).to(dev) for a in (wl.omega, wl.thx, wl.thy)]
-    src = wl.batch if wl.batch is not None else wl.traj
-    pinned = {k: torch.from_numpy(np.ascontiguousarray(v)).pin_memory() for k, v in src.items()}
-    dtr = {k: v.to(dev) for k, v in pinned.items()}
-    count = len(wl.n) if wl.batch is not None else 1
-    n_max = int(np.max(wl.n)) if wl.batch is not None else len(wl.traj["t"])
-    ws = torch.empty(rad.rad_workspace_bytes(count, n_max, len(wl.omega), len(wl.thx), len(wl.thy)),
-                     dtype=torch.uint8, device=dev)
-    out = torch.empty((len(wl.omega), len(wl.thy), len(wl.thx)), dtype=torch.float64, device=dev)
-    lam_vec = np.full(count, lam) if model else None
+    def to_dev(self, a):
+        return self.torch.from_numpy(np.ascontiguousarray(a)).to(self.dev)
 
-    def step():
+    # ---- one workload, device-resident: W untimed steps, K timed ones
+    def run(self, wl, steps, warmup, kernel=0, shard=None):
+        """shard: None (whole job on this rank), "omega" (grid sharded across ranks), "ensemble" (trajectories dealt
+        out, one exchange inside the timed region)."""
+        torch, rad = self.torch, self.rad
+        from paper_1910_10391_b200.sharding import shard_range
+        model, lam = wl.model, wl.hbarc_over_E
+        omega, thx, thy = (self.to_dev(a) for a in (wl.omega, wl.thx, wl.thy))
+        n_w = len(wl.omega)
+        if shard == "omega":
+            lo, hi = shard_range(n_w, self.rank, self.world)
+            omega = omega[lo:hi].contiguous()
+            n_w = hi - lo
         if wl.batch is not None:
-            rad.rad_ensemble_sum(dtr, wl.n, *grid, model=model, hbarc_over_E=lam_vec, out=out, workspace=ws)
-        elif model == 0:
-            rad.rad_classical(dtr, *grid, out=out, workspace=ws)
+            p_lo, p_hi = shard_range(len(wl.n), self.rank, self.world) if shard == "ensemble" else (0, len(wl.n))
+            dtr = {k: self.to_dev(v[p_lo:p_hi]) for k, v in wl.batch.items()}
+            n_vec = np.ascontiguousarray(wl.n[p_lo:p_hi])
+            count, n_max = len(n_vec), int(np.max(n_vec)) if len(n_vec) else 2
         else:
-            rad.rad_semiclassical(dtr, *grid, 0 if model == 1 else 1, lam, out=out, workspace=ws)
+            dtr = {k: self.to_dev(v) for k, v in wl.traj.items()}
+            n_vec, count, n_max = None, 1, len(wl.traj["t"])
+        ws = torch.empty(max(256, rad.rad_workspace_bytes(max(count, 1), n_max, max(n_w, 1), len(wl.thx), len(wl.thy))),
+                         dtype=torch.uint8, device=self.dev)
+        out = torch.empty((max(n_w, 1), len(wl.thy), len(wl.thx)), dtype=torch.float64, device=self.dev)
+        lam_vec = np.full(max(count, 1), lam) if model else None
+        parts = torch.empty((self.world, *out.shape), dtype=torch.float64, device=self.dev) if shard == "ensemble" else None
+        total = torch.empty_like(out) if shard == "ensemble" else None
 
-    flush = torch.empty(256 << 20, dtype=torch.uint8, device=dev)      # > 126 MB L2
+        def step():
+            if n_w == 0 or count == 0:
+                out.zero_()
+            elif wl.batch is not None:
+                rad.rad_ensemble_sum(dtr, n_vec, omega, thx, thy, model=model, hbarc_over_E=lam_vec, out=out, workspace=ws,
+                                     kernel=kernel, profile=self.prof)
+            elif model == 0:
+                rad.rad_classical(dtr, omega, thx, thy, out=out, workspace=ws, kernel=kernel, profile=self.prof)
+            else:
+                rad.rad_semiclassical(dtr, omega, thx, thy, 0 if model == 1 else 1, lam, out=out, workspace=ws,
+                                      kernel=kernel, profile=self.prof)
+            if shard == "ensemble" and self.world > 1:                 # the ONE exchange of SURVEY.md 8(e)(ii)
+                self.dist.all_gather_into_tensor(parts.view(-1), out.view(-1))
+                rad.rad_sum_cubes(parts, out=total)
 
-    def barrier():
-        if world > 1:
-            dist.barrier()
-        torch.cuda.synchronize()
-
-    peak = rad.rad_measure_fp64_peak(300.0)                            # FLOP/s, measured here
-    rad.rad_profile_enable(True)
-    rad.rad_set_kernel({"auto": 0, "direct": 1, "separable": 2}[args.kernel])
-    kernel = rad.rad_plan_kernel(len(wl.omega), len(wl.thx), len(wl.thy), model)
-
-    def timed_steps(n_steps):
-        """W untimed steps, then n_steps timed ones: (sum of step ms, per-step main-kernel ms, launches, clocks)."""
-        for _ in range(max(args.warmup, 3)):
-            flush.zero_()
+        for _ in range(warmup):
+            self.flush.zero_()
             step()
-        barrier()
-        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True))
-              for _ in range(n_steps)]
-        kernel_ms = []
+        self.barrier()
+        ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(steps)]
         launches0 = rad.rad_launch_count()
-        with ClockSampler(local) as clk:
-            for a, b in ev:
-                flush.zero_()
+        with ClockSampler(self.local) as clk:
+            for a, b in ev:                                            # no host synchronisation inside the timed region
+                self.flush.zero_()
                 a.record()
                 step()
                 b.record()
-                kernel_ms.append(rad.rad_profile_last()[1])            # waits for this step
             torch.cuda.synchronize()
-        n_launch = rad.rad_launch_count() - launches0
-        barrier()
-        return sum(a.elapsed_time(b) for a, b in ev), kernel_ms, n_launch, clk
+        launches = rad.rad_launch_count() - launches0
+        self.barrier()
+        total_ms = sum(a.elapsed_time(b) for a, b in ev)
+        main_ms = []                                                   # the main kernel's own duration: a few extra
+        for _ in range(min(steps, 3) if n_w and count else 0):         # steps, each read back (this synchronises)
+            self.flush.zero_()
+            step()
+            main_ms.append(self.prof.read()[1])
+        rank_ms = total_ms
+        if self.world > 1:
+            t = torch.tensor([total_ms], dtype=torch.float64, device=self.dev)
+            all_t = [torch.empty_like(t) for _ in range(self.world)]
+            self.dist.all_gather(all_t, t)
+            rank_ms = [float(x.item()) / steps for x in all_t]
+            total_ms = max(float(x.item()) for x in all_t)
+        plan = rad.rad_plan_describe(max(count, 1), n_max, max(n_w, 1), len(wl.thx), len(wl.thy), model, kernel)
+        return {"wl": wl, "steps": steps, "warmup": warmup, "total_ms": total_ms, "main_ms": main_ms, "launches": launches,
+                "clocks": clk.summary(), "plan": plan, "rank_ms_per_step": rank_ms, "local_points": n_w * len(wl.thx) * len(wl.thy),
+                "local_samples": int(np.sum(n_vec)) if n_vec is not None else n_max, "shard": shard}
 
-    total_ms, main_ms, launches, clocks = timed_steps(args.steps)
+    # ---- roofline of a run: algorithmic flops of the kernels that ran / the main kernels' own time
+    def roofline(self, r):
+        wl, plan = r["wl"], r["plan"]
+        model = wl.model
+        evals = float(r["local_points"]) * r["local_samples"]          # this rank's evals per step
+        if not r["main_ms"] or evals == 0:
+            return None
+        main_s = float(np.mean(r["main_ms"])) * 1e-3
+        k = plan["kernel"]
+        if plan["parts"] == 2:                                         # separable interior + direct rest
+            frac_sep = plan["interior_x"] * plan["interior_y"] / (len(wl.thx) * len(wl.thy))
+            flops = evals * (frac_sep * FLOPS_PER_EVAL[2][model] + (1 - frac_sep) * FLOPS_PER_EVAL[1][model])
+            instr = evals * (frac_sep * FP64_INSTR_PER_EVAL[2][model] + (1 - frac_sep) * FP64_INSTR_PER_EVAL[1][model])
+            name = f"{KERNELS[2]} on {plan['interior_x']} x {plan['interior_y']} angles + {KERNELS[1]} on the rest"
+        else:
+            flops, instr, name = evals * FLOPS_PER_EVAL[k][model], evals * FP64_INSTR_PER_EVAL[k][model], KERNELS[k]
+        achieved = flops / main_s
+        key = f"{wl.name}|{k}"
+        return {"bound": "alu", "kernel": name, "achieved": achieved / 1e12, "peak": self.peak / 1e12, "unit": "TFLOP/s",
+                "frac": achieved / self.peak,
+                "traffic": self.traffic.get(key),
+                "traffic_unit": "bytes per main-kernel launch (ncu --set full capture under profiles/, not this run)",
+                "peak_kind": "FP64 FMA microbenchmark measured in this run (rad_measure_fp64_peak)",
+                "peak_spec": FP64_SPEC_TFLOPS, "frac_of_spec": achieved / 1e12 / FP64_SPEC_TFLOPS,
+                "flops_per_eval": flops / evals, "fp64_issue_frac": instr / main_s / (self.peak / 2.0),
+                "main_kernel_ms": main_s * 1e3,
+                "main_kernel_share_of_step": main_s * 1e3 / (float(np.mean(r["rank_ms_per_step"])) if isinstance(r["rank_ms_per_step"], list)
+                                                             else r["total_ms"] / r["steps"])}
 
-    # the same workload through the other (direct-phasor) kernel, for the record: the north_star
-    # target (>= 60 % of FP64 peak) is stated for the kernel that evaluates one phasor per eval
-    direct = None
-    if kernel == 2 and args.kernel == "auto" and rank == 0 and world == 1 and total_ms / args.steps < 2000.0:
-        rad.rad_set_kernel(1)
-        d_total, d_main, _, _ = timed_steps(min(args.steps, 5))
-        rad.rad_set_kernel(0)
-        d_s = float(np.mean(d_main)) * 1e-3
-        d_flops = FLOPS_PER_EVAL[1][model] * wl.evals / d_s
-        direct = {"kernel": KERNELS[1], "value": wl.evals * min(args.steps, 5) / (d_total * 1e-3), "unit": UNIT,
-                  "main_kernel_ms": d_s * 1e3, "flops_per_eval": FLOPS_PER_EVAL[1][model],
-                  "achieved": d_flops / 1e12, "frac": d_flops / peak,
-                  "fp64_issue_frac": FP64_INSTR_PER_EVAL[1][model] * wl.evals / d_s / (peak / 2.0)}
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
-    evals_step = wl.evals
-    value = world * evals_step * args.steps / (total_ms * 1e-3)
+    def entry(self, r, with_direct=None):
+        """per_config record of a run (value = whole-job evals/s)."""
+        wl = r["wl"]
+        e = {"workload": wl.name, "model": MODELS[wl.model], "evals_per_step": wl.evals,
+             "value": wl.evals * r["steps"] / (r["total_ms"] * 1e-3), "unit": UNIT,
+             "ms_per_step": r["total_ms"] / r["steps"], "steps": r["steps"], "warmup": r["warmup"],
+             "launches_per_step": r["launches"] / r["steps"], "plan": r["plan"], "roofline": self.roofline(r),
+             "clocks": r["clocks"]}
+        if r["shard"]:
+            e["sharding"] = r["shard"]
+            e["rank_ms_per_step"] = r["rank_ms_per_step"]
+        if with_direct is not None:
+            d = with_direct
+            e["direct_kernel_same_run"] = {"value": wl.evals * d["steps"] / (d["total_ms"] * 1e-3), "unit": UNIT,
+                                           "ms_per_step": d["total_ms"] / d["steps"], "steps": d["steps"],
+                                           "warmup": d["warmup"], "roofline": self.roofline(d)}
+        return e
 
     # ---- end to end through the host-buffer C-ABI call (pinned inputs, H2D + D2H inside)
-    host_out = torch.empty(out.shape, dtype=torch.float64).pin_memory()
-    host_grid = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (wl.omega, wl.thx, wl.thy)]
+    def e2e(self, wl, steps, kernel):
+        torch, rad = self.torch, self.rad
+        src = wl.batch if wl.batch is not None else wl.traj
+        pinned = {k: torch.from_numpy(np.ascontiguousarray(v)).pin_memory() for k, v in src.items()}
+        host_grid = [torch.from_numpy(np.ascontiguousarray(a)).pin_memory() for a in (wl.omega, wl.thx, wl.thy)]
+        host_out = torch.empty((len(wl.omega), len(wl.thy), len(wl.thx)), dtype=torch.float64).pin_memory()
+        lam_vec = np.full(len(wl.n), wl.hbarc_over_E) if wl.batch is not None and wl.model else None
 
-    def e2e_step():
-        if wl.batch is not None:
-            rad.rad_ensemble_sum_host(pinned, wl.n, *host_grid, model=model, hbarc_over_E=lam_vec, out=host_out)
-        else:
-            rad.rad_eval_host(pinned, *host_grid, model, lam, out=host_out)
+        def step():
+            if wl.batch is not None:
+                rad.rad_ensemble_sum_host(pinned, wl.n, *host_grid, model=wl.model, hbarc_over_E=lam_vec, out=host_out,
+                                          kernel=kernel)
+            else:
+                rad.rad_eval_host(pinned, *host_grid, wl.model, wl.hbarc_over_E, out=host_out, kernel=kernel)
 
-    e2e_steps = max(3, min(args.steps, 10))
-    for _ in range(2):
-        e2e_step()
-    barrier()
-    t0 = time.perf_counter()
-    for _ in range(e2e_steps):
-        flush.zero_()
-        torch.cuda.synchronize()
-        e2e_step()                                                     # returns after D2H completed
-    e2e_wall = time.perf_counter() - t0
-    # subtract nothing: the flush is inside this wall-clock region, so time it separately
-    torch.cuda.synchronize()
-    t1 = time.perf_counter()
-    for _ in range(e2e_steps):
-        flush.zero_()
-        torch.cuda.synchronize()
-    flush_wall = time.perf_counter() - t1
-    e2e_t = torch.tensor([e2e_wall - flush_wall], dtype=torch.float64, device=dev)
+        for _ in range(2 if wl.evals < 1e12 else 1):
+            step()
+        self.barrier()
+        wall = 0.0
+        for _ in range(steps):
+            self.flush.zero_()
+            torch.cuda.synchronize()
+            t0 = time.perf_counter()
+            step()                                                     # returns after D2H completed
+            wall += time.perf_counter() - t0
+        h2d = sum(v.numel() * 8 for v in pinned.values()) + sum(g.numel() * 8 for g in host_grid)
+        return wl.evals * steps / wall, h2d, host_out.numel() * 8, steps
+
+
+def run_b200(args):
+    B = Bench(args)
+    world, rank = B.world, B.rank
+    kopt = {"auto": 0, "direct": 1, "separable": 2, "fused": 3}[args.kernel]
+    wl = make_workload(args.workload, args.cfg4_count, args.spin)
+    shard = None
     if world > 1:
-        dist.all_reduce(e2e_t, op=dist.ReduceOp.MAX)
-    e2e_value = world * evals_step * e2e_steps / float(e2e_t.item())
-    h2d = sum(v.numel() * 8 for v in pinned.values()) + sum(g.numel() * 8 for g in host_grid)
-    d2h = host_out.numel() * 8
+        shard = "ensemble" if wl.batch is not None else "omega"
+    warmup = max(args.warmup, 3)
+    head = B.run(wl, args.steps, warmup, kopt, shard)
+    step_ms = head["total_ms"] / args.steps
+    value = wl.evals * args.steps / (head["total_ms"] * 1e-3)
+
+    # the same workload through the direct (one phasor per eval) kernel, for the record: the north_star target
+    # (>= 60 % of FP64 peak) is stated for that kernel
+    direct = None
+    if head["plan"]["kernel"] == 2 and args.kernel == "auto" and world == 1:
+        few = 5 if step_ms < 500 else 2
+        direct = B.run(wl, few, 3 if step_ms < 500 else 1, 1)
+
+    e2e_value = e2e_info = None
+    if world == 1:
+        e2e_steps = max(3, min(args.steps, 10)) if step_ms < 1000 else 3
+        e2e_value, h2d, d2h, e2e_steps = B.e2e(wl, e2e_steps, kopt)
+        e2e_info = {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
+                    "steps": e2e_steps, "call": "rad_eval_host / rad_ensemble_sum_host (pinned host buffers)"}
+    else:
+        e2e_info = {"value": None, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0,
+                    "note": "host-buffer entry points are single-GPU calls; measured at --gpus 1"}
+
+    per_config = []
+    if not args.no_per_config and args.workload == "cfg5" and args.spin == "1/2" and args.kernel == "auto":
+        # (workload, spin, timed steps, warm-up, also time the direct kernel?)
+        todo = [("cfg2", "1/2", 20, 3, True), ("cfg3", "1/2", 5, 3, True), ("cfg4", "1/2", 2, 1, False),
+                ("cfg5", "0", 2, 1, False), ("cfg1", "1/2", 50, 5, True), ("paper_typical", "1/2", 20, 3, True)]
+        for name, spin, k, w, with_direct in todo:
+            w2 = make_workload(name, args.cfg4_count, spin)
+            sh = None
+            if world > 1:
+                sh = "ensemble" if w2.batch is not None else "omega"
+            r = B.run(w2, k, w, 0, sh)
+            d = B.run(w2, min(k, 5), min(w, 3), 1) if with_direct and world == 1 and r["plan"]["kernel"] != 1 else None
+            per_config.append(B.entry(r, d))
+            del w2, r, d
+            B.torch.cuda.empty_cache()
 
     if rank == 0:
-        main_s = float(np.mean(main_ms)) * 1e-3
-        achieved = FLOPS_PER_EVAL[kernel][model] * evals_step / main_s
+        n_max = int(np.max(wl.n)) if wl.batch is not None else len(wl.traj["t"])
+        count = len(wl.n) if wl.batch is not None else 1
+        roof = B.roofline(head)
+        if direct is not None and roof is not None:
+            roof["direct_kernel_same_run"] = {"kernel": KERNELS[1], "value": wl.evals * direct["steps"] / (direct["total_ms"] * 1e-3),
+                                              "unit": UNIT, "steps": direct["steps"], "warmup": direct["warmup"],
+                                              **{k: v for k, v in B.roofline(direct).items()
+                                                 if k in ("achieved", "frac", "flops_per_eval", "fp64_issue_frac", "main_kernel_ms")}}
+        par = {None: "one GPU", "omega": f"grid sharded in {world} omega slabs, whole trajectory on every rank, no exchange in the computation",
+               "ensemble": f"trajectories dealt out to {world} ranks; all-gather of partial cubes + ordered sum inside the timed region"}[shard]
         line = {
             "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps,
-            "warmup": max(args.warmup, 3), "ms_per_step": total_ms / args.steps,
-            "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+            "warmup": warmup, "ms_per_step": step_ms,
+            "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
-            "config": {"workload": wl.name, "model": ["classical", "spin0", "spin1/2"][model],
-                       "samples": n_max, "trajectories": count,
-                       "grid": [len(wl.omega), len(wl.thy), len(wl.thx)], "evals_per_step": evals_step,
-                       "l2": "flushed between steps (256 MiB memset)",
-                       "parallelism": f"replicas x{world}, one trajectory per rank, no collective"},
-            "clocks": clocks.summary(),
-            "e2e": {"value": e2e_value, "unit": UNIT, "h2d_bytes_per_step": h2d, "d2h_bytes_per_step": d2h,
-                    "steps": e2e_steps, "call": "rad_eval_host / rad_ensemble_sum_host (pinned host buffers)"},
-            "gpu_launches": int(launches),
-            "roofline": {"bound": "alu", "kernel": KERNELS[kernel],
-                         "achieved": achieved / 1e12, "peak": peak / 1e12, "unit": "TFLOP/s",
-                         "frac": achieved / peak,
-                         "traffic": NCU_TRAFFIC_BYTES.get((args.workload, kernel)) if args.spin == "1/2" else None,
-                         "traffic_unit": "bytes per main-kernel launch (ncu capture in profiles/, not this run)",
-                         "peak_kind": "FP64 FMA microbenchmark measured in this run (rad_measure_fp64_peak)",
-                         "peak_spec": FP64_SPEC_TFLOPS, "frac_of_spec": achieved / 1e12 / FP64_SPEC_TFLOPS,
-                         "flops_per_eval": FLOPS_PER_EVAL[kernel][model],
-                         "fp64_issue_frac": FP64_INSTR_PER_EVAL[kernel][model] * evals_step / main_s / (peak / 2.0),
-                         "main_kernel_ms": main_s * 1e3,
-                         "main_kernel_share_of_step": main_s * 1e3 / (total_ms / args.steps)},
+            "config": {"workload": wl.name, "model": MODELS[wl.model], "samples": n_max, "trajectories": count,
+                       "grid": [len(wl.omega), len(wl.thy), len(wl.thx)], "evals_per_step": wl.evals,
+                       "l2": "flushed between steps (256 MiB memset)", "parallelism": par, "plan": head["plan"]},
+            "clocks": head["clocks"],
+            "e2e": e2e_info,
+            "gpu_launches": int(head["launches"]),
+            "roofline": roof,
         }
-        if direct is not None:
-            line["roofline"]["direct_kernel_same_run"] = direct
+        if world > 1:
+            line["rank_ms_per_step"] = head["rank_ms_per_step"]
+        if per_config:
+            line["per_config"] = per_config
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = cpu_baseline(wl)
         print(json.dumps(line))
     if world > 1:
-        dist.destroy_process_group()
+        B.dist.destroy_process_group()
     return 0
 
 

@@ -243,7 +243,10 @@ __device__ __forceinline__ dd half_theta2_dd(double nx, double ny) {
 
 // ------------------------------------------------------------------------------ main (a0-a5)
 // NC = number of real accumulators per omega: 4 (A_x, A_y) or 6 (+ J, spin-1/2).
-template <int NC, int DEG>
+// GEN: the general instantiation -- angles on the L-shaped rest of a two-part plan and / or the angular-spectrum
+// epilogue.  The plain one (cube on a whole tensor grid) is what the BASELINE configs run; the extra index
+// arithmetic of the general one costs it registers (255 + spills with 6 accumulators per omega: -30 % measured).
+template <int NC, int DEG, bool GEN>
 __global__ void __launch_bounds__(TPB, 1)
 rad_main_kernel(const MainParams P) {
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -261,8 +264,8 @@ rad_main_kernel(const MainParams P) {
     const int wg = (int)(gc / A), a = (int)(gc % A);
     double nx, ny;
     {
-        int ix, iy;
-        angle_of(P, a, ix, iy);
+        int ix = a % P.n_thx, iy = a / P.n_thx;
+        if (GEN) angle_of(P, a, ix, iy);
         nx = P.thx[ix]; ny = P.thy[iy];
     }
     const dd h = half_theta2_dd(nx, ny);               // theta^2 / 2, double-double
@@ -376,7 +379,7 @@ rad_main_kernel(const MainParams P) {
         double *dst = P.partial + (int64_t)slice * W * P.t_pad + gid;
 #pragma unroll
         for (int j = 0; j < W; ++j) dst[(int64_t)j * P.t_pad] = S_sum[j];
-    } else if (P.mode == MODE_DIRECT && P.ang) {
+    } else if (GEN && P.ang && P.mode == MODE_DIRECT) {
         // ---- angular spectrum: sum of this CTA's angles per omega, in thread order (N1)
         __syncthreads();                              // the ring is free: every chunk has been consumed
         double *red = ring;                           // [TPB][W]
@@ -394,8 +397,8 @@ rad_main_kernel(const MainParams P) {
             P.ang_partial[((int64_t)blockIdx.x * P.ang_groups + g) * W + j] = sum;
         }
     } else if (P.mode == MODE_DIRECT && gid < T) {
-        int ix, iy;                                   // (recomputed: not kept in registers across the time loop)
-        angle_of(P, a, ix, iy);
+        int ix = a % P.n_thx, iy = a / P.n_thx;       // (recomputed: not kept in registers across the time loop)
+        if (GEN) angle_of(P, a, ix, iy);
 #pragma unroll
         for (int j = 0; j < W; ++j) {
             const int iw = wg * W + j;
@@ -657,9 +660,15 @@ static CallPlan plan_for(int count, int64_t n_max, int n_omega, int n_thx, int n
 
 template <int NC, int DEG>
 static cudaError_t launch_main(const MainParams &mp, dim3 grid, cudaStream_t st) {
-    const cudaError_t a = ensure_smem(rad_main_kernel<NC, DEG>, NC == 6 ? 1 : 0, SMEM_BYTES);
-    if (a != cudaSuccess) return a;
-    rad_main_kernel<NC, DEG><<<grid, TPB, SMEM_BYTES, st>>>(mp);
+    if (mp.ang || mp.l_x0 >= 0) {
+        const cudaError_t a = ensure_smem(rad_main_kernel<NC, DEG, true>, NC == 6 ? 5 : 4, SMEM_BYTES);
+        if (a != cudaSuccess) return a;
+        rad_main_kernel<NC, DEG, true><<<grid, TPB, SMEM_BYTES, st>>>(mp);
+    } else {
+        const cudaError_t a = ensure_smem(rad_main_kernel<NC, DEG, false>, NC == 6 ? 1 : 0, SMEM_BYTES);
+        if (a != cudaSuccess) return a;
+        rad_main_kernel<NC, DEG, false><<<grid, TPB, SMEM_BYTES, st>>>(mp);
+    }
     ++g_launches;
     return cudaGetLastError();
 }

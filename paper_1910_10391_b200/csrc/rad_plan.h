@@ -159,7 +159,7 @@ static inline void choose_parts(int n_omega, int n_thx, int n_thy, int nc, int k
 
 // The fused single-launch kernel: one trajectory, direct-kernel arithmetic, every CTA resident at once
 // (cooperative launch).  Tiles of FUSED_TPB threads x PLAN_W omegas; the time axis is cut into as many slices as
-// fill `resident` CTAs (at least FUSED_SUB samples each).
+// fill `resident` CTAs (at least 32 samples each).
 static inline bool fused_applies(int count, int64_t n_max, int n_omega, int n_thx, int n_thy, int resident,
                                  int &tiles, int &slices) {
     if (count != 1 || resident <= 0) return false;
@@ -167,7 +167,9 @@ static inline bool fused_applies(int count, int64_t n_max, int n_omega, int n_th
     const int64_t t64 = (T + FUSED_TPB - 1) / FUSED_TPB;
     if (t64 > resident) return false;
     tiles = (int)t64;
-    const int64_t max_by_samples = std::max<int64_t>(1, n_max / FUSED_SUB);
+    // at least 32 samples per slice: below that the per-CTA prologue (omega* as double-doubles, base phases)
+    // is no longer small against the samples it serves
+    const int64_t max_by_samples = std::max<int64_t>(1, n_max / 32);
     slices = (int)std::max<int64_t>(1, std::min<int64_t>(resident / tiles, max_by_samples));
     return true;
 }

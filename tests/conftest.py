@@ -14,6 +14,7 @@ os.environ.setdefault("OMP_NUM_THREADS", str(os.cpu_count() or 1))
 
 def pytest_configure(config):
     config.addinivalue_line("markers", "gpu: needs a CUDA device (run on the B200 box)")
+    config.addinivalue_line("markers", "multigpu: needs two CUDA devices and NCCL (skipped, with that reason, on one)")
 
 
 @pytest.fixture(scope="session")
