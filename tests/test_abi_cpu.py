@@ -144,8 +144,8 @@ def test_launch_plans_of_the_baseline_configs(radlib):
     if torch.cuda.is_available():
         pytest.skip("plan depends on the visible device's SM count; this checks the 148-SM default")
     d = radlib.rad_plan_describe
-    p = d(1, 4000, 64, 8, 8, 0)                      # cfg 1: fused kernel, 8 tiles of 64 threads x 62 time slices, ONE launch
-    assert (p["kernel"], p["tiles"], p["slices"], p["launches"]) == (3, 8, 62, 1)
+    p = d(1, 4000, 64, 8, 8, 0)                      # cfg 1: fused kernel, 8 tiles of 64 threads x 74 time slices = 592 resident CTAs, ONE launch
+    assert (p["kernel"], p["tiles"], p["slices"], p["launches"]) == (3, 8, 74, 1)
     assert p["tiles"] * p["slices"] <= 4 * 148
     p = d(1, 4000, 64, 8, 8, 0, kernel=1)            # the three-launch direct path: 4 tiles x 32 one-chunk time slices
     assert (p["kernel"], p["mode"], p["tiles"], p["slices"], p["chunks"], p["launches"]) == (1, 2, 4, 32, 32, 3)
