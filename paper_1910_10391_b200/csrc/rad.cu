@@ -65,6 +65,7 @@ struct MainParams {
     int ang, ang_groups;      // ang_groups: omega groups a CTA of the direct kernel can span
     double cut2;              // theta_cut^2, <= 0: no mask
     double *ang_partial;
+    int cl;                   // separable kernel: 2 = launched as cluster pairs that share the T table, else 1
 };
 
 // Angles a launch of the direct kernel covers, and the (i_x, i_y) of its a-th angle.
@@ -675,9 +676,22 @@ static cudaError_t launch_main(const MainParams &mp, dim3 grid, cudaStream_t st)
 
 template <int NC, int WY>
 static cudaError_t launch_sep(const MainParams &mp, dim3 grid, cudaStream_t st) {
-    const cudaError_t a = ensure_smem(rad_sep_kernel<NC, WY>, NC == 6 ? 3 : 2, SepShape<NC, WY>::SMEM);
+    if (mp.cl == 2) {         // cluster pairs along the y tiles (thread-block cluster of 2 CTAs on neighbouring SMs)
+        const cudaError_t a = ensure_smem(rad_sep_kernel<NC, WY, 2>, NC == 6 ? 7 : 6, SepShape<NC, WY>::SMEM);
+        if (a != cudaSuccess) return a;
+        cudaLaunchConfig_t cfg = {};
+        cfg.gridDim = grid; cfg.blockDim = dim3(SepRegs<NC>::THREADS); cfg.dynamicSmemBytes = SepShape<NC, WY>::SMEM;
+        cfg.stream = st;
+        cudaLaunchAttribute at[1];
+        at[0].id = cudaLaunchAttributeClusterDimension;
+        at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
+        cfg.attrs = at; cfg.numAttrs = 1;
+        ++g_launches;
+        return cudaLaunchKernelEx(&cfg, rad_sep_kernel<NC, WY, 2>, mp);
+    }
+    const cudaError_t a = ensure_smem(rad_sep_kernel<NC, WY, 1>, NC == 6 ? 3 : 2, SepShape<NC, WY>::SMEM);
     if (a != cudaSuccess) return a;
-    rad_sep_kernel<NC, WY><<<grid, SepRegs<NC>::THREADS, SepShape<NC, WY>::SMEM, st>>>(mp);
+    rad_sep_kernel<NC, WY, 1><<<grid, SepRegs<NC>::THREADS, SepShape<NC, WY>::SMEM, st>>>(mp);
     ++g_launches;
     return cudaGetLastError();
 }
@@ -793,6 +807,13 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const int64
         mp.partial = reinterpret_cast<double *>(ws + pt.off_partial);
         mp.t_pad = pl.t_pad;
         mp.l_x0 = pt.l_x0; mp.l_y0 = pt.l_y0;
+        mp.cl = 1;
+#ifndef RAD_SEP_NO_CLUSTER
+        if (pt.kernel == K_SEP) {                     // an even number of y tiles: cluster pairs share the T table
+            const int ty = nc == 6 ? 8 : 16;
+            if (((pt.n_thy + ty - 1) / ty) % 2 == 0) mp.cl = 2;
+        }
+#endif
         if (ang) {
             mp.ang = 1; mp.cut2 = ang->cut2;
             mp.ang_groups = std::min((g->n_omega + W - 1) / W, (TPB + pt.angles - 1) / pt.angles + 1);

@@ -102,11 +102,20 @@ struct SepCoord {
     int bw, bx, by;                  // first omega / x / y index of the CTA tile
     int iw0, ix0, iy0;               // first omega / x / y index of this thread's points
     int lw, lx, ly, ww, wx;
-    __device__ __forceinline__ SepCoord(int block, int tid, int n_thx, int n_thy) {
+    // cl = 2: the CTAs of a cluster pair (blocks 2k, 2k + 1) own neighbouring y tiles of one (omega, x) tile,
+    // so that they share the T table (rad_sep_kernel); the y tile count is even then.
+    __device__ __forceinline__ SepCoord(int block, int tid, int n_thx, int n_thy, int cl) {
         const int ntx = (n_thx + 15) / 16, nty = (n_thy + 4 * WY - 1) / (4 * WY);
-        bx = (block % ntx) * 16;
-        by = ((block / ntx) % nty) * 4 * WY;
-        bw = (block / (ntx * nty)) * 16;
+        if (cl == 2) {
+            const int rest = block >> 1, half = nty >> 1;
+            bx = (rest % ntx) * 16;
+            by = (((rest / ntx) % half) * 2 + (block & 1)) * 4 * WY;
+            bw = (rest / (ntx * half)) * 16;
+        } else {
+            bx = (block % ntx) * 16;
+            by = ((block / ntx) % nty) * 4 * WY;
+            bw = (block / (ntx * nty)) * 16;
+        }
         const int lane = tid & 31, warp = tid >> 5;
         lw = lane & 1; ly = (lane >> 1) & 3; lx = (lane >> 3) & 3;
         ww = warp >> 1; wx = warp & 1;
@@ -165,6 +174,33 @@ template <int REGS> __device__ __forceinline__ void reg_alloc() {
 template <int REGS> __device__ __forceinline__ void reg_dealloc() {
     asm volatile("setmaxnreg.dec.sync.aligned.u32 %0;" ::"n"(REGS));
 }
+// ---- cluster pair (CL = 2): distributed shared memory and cluster-scope barriers
+__device__ __forceinline__ uint32_t cluster_ctarank() {
+    uint32_t r;
+    asm volatile("mov.u32 %0, %%cluster_ctarank;" : "=r"(r));
+    return r;
+}
+__device__ __forceinline__ uint32_t map_to_cta(uint32_t smem_addr, uint32_t rank) {   // same offset in CTA `rank`
+    uint32_t r;
+    asm volatile("mapa.shared::cluster.u32 %0, %1, %2;" : "=r"(r) : "r"(smem_addr), "r"(rank));
+    return r;
+}
+// asynchronous 16-byte store into the peer CTA's shared memory; its completion is counted in bytes on the peer's
+// mbarrier `bar` (both shared::cluster addresses) -- no fence on either side: the data has landed when the
+// barrier's transaction count says so
+__device__ __forceinline__ void st_async_v2(uint32_t addr, double2 v, uint32_t bar) {
+    asm volatile("st.async.weak.shared::cluster.mbarrier::complete_tx::bytes.v2.f64 [%0], {%1, %2}, [%3];"
+                 ::"r"(addr), "d"(v.x), "d"(v.y), "r"(bar) : "memory");
+}
+// arrive on a barrier of the peer CTA (consumer release of a table buffer: nothing to publish, program order
+// keeps the arrive behind the loads whose values the warp has already used)
+__device__ __forceinline__ void mbar_arrive_remote(uint32_t addr) {
+    asm volatile("mbarrier.arrive.shared::cluster.b64 _, [%0];" ::"r"(addr) : "memory");
+}
+__device__ __forceinline__ void cluster_sync_all() {
+    asm volatile("barrier.cluster.arrive.release.aligned;" ::: "memory");
+    asm volatile("barrier.cluster.wait.acquire.aligned;" ::: "memory");
+}
 template <int NPROD> __device__ __forceinline__ void producer_bar_sync() {   // named barrier 1: the producer threads
     asm volatile("bar.sync 1, %0;" ::"n"(NPROD) : "memory");
 }
@@ -217,9 +253,17 @@ struct SepCursor {
 };
 
 // ------------------------------------------------------------------------------ main (a0-a7)
-template <int NC, int WY>
+// CL = 2: launched as clusters of two CTAs that own neighbouring y tiles of one (omega, x) tile.  Their T tables are
+// identical, so each CTA's producers compute HALF of the T entries and store them into both CTAs' table rings: the
+// local half with an ordinary store, the peer's with st.async, whose bytes the peer's full[] barrier counts
+// (expect_tx posted with the arrival of the peer's first producer warp).  empty[] counts the consumer warps of both
+// CTAs, so a producer overwrites a buffer only when both CTAs have read it.  Y, F, H stay private.  Both CTAs step through the same (trajectory, chunk,
+// sub-block) sequence, so the protocol is symmetric; a cluster barrier at the start (barriers initialised before the
+// peer arrives on them) and at the end (no CTA leaves while the peer may still store into it) frames it.
+template <int NC, int WY, int CL>
 __global__ void __launch_bounds__(SepRegs<NC>::THREADS, 1)
 rad_sep_kernel(const MainParams P) {
+    static_assert(CL == 1 || CL == 2, "cluster pair or single CTA");
     using SH = SepShape<NC, WY>;
     constexpr int YN = SH::YN, EV = SH::EV, S = SEP_S, NB = SEP_NB;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -235,30 +279,39 @@ rad_sep_kernel(const MainParams P) {
 
     if (tid == 0) {
         for (int s = 0; s < SEP_STAGES; ++s) mbar_init(&bars[s], 1);
-        for (int b = 0; b < NB; ++b) { mbar_init(&full[b], SepRegs<NC>::NPROD / 32); mbar_init(&empty[b], SEP_CONS / 32); }
+        for (int b = 0; b < NB; ++b) { mbar_init(&full[b], SepRegs<NC>::NPROD / 32); mbar_init(&empty[b], CL * SEP_CONS / 32); }
         mbar_fence_init();
     }
     __syncthreads();
+    uint32_t peer = 0, my_rank = 0;
+    if (CL == 2) {
+        cluster_sync_all();                           // the peer's barriers are initialised
+        my_rank = cluster_ctarank();
+        peer = my_rank ^ 1u;
+    }
 
     if (tid >= SEP_CONS) {
         // ====================================================================== PRODUCERS (phase A)
         reg_dealloc<SepRegs<NC>::PROD>();
         const int pt = tid - SEP_CONS;
         const int tile_bx = blockIdx.x;
-        const SepCoord<WY> co(tile_bx, 0, P.n_thx, P.n_thy);             // tile bases only
+        const SepCoord<WY> co(tile_bx, 0, P.n_thx, P.n_thy, CL);         // tile bases only
         // Entries per thread and sample.  T: 256 / NPROD.  Y and F: YN / NPROD each, or -- when there are more
         // producer threads than Y entries -- one Y entry for threads [0, YN) and one F entry for the rest
         // (whole warps take one role: YN is a multiple of 32).
         constexpr int NPROD = SepRegs<NC>::NPROD;
         constexpr bool SPLIT = YN < NPROD;
         static_assert(256 % NPROD == 0 && (SPLIT ? 2 * YN == NPROD : YN % NPROD == 0), "producer entry assignment");
-        constexpr int RT = 256 / NPROD, RY = SPLIT ? 1 : YN / NPROD;
+        static_assert((256 / NPROD) % CL == 0, "the T entries of a thread are dealt out to the CTAs of the pair");
+        constexpr int RT = 256 / NPROD / CL, RY = SPLIT ? 1 : YN / NPROD;   // CL = 2: entry slots r * CL + rank
         const bool doY = !SPLIT || pt < YN, doF = !SPLIT || pt >= YN;
         const int ptF = SPLIT ? (pt >= YN ? pt - YN : 0) : pt, ptY = SPLIT ? (pt < YN ? pt : 0) : pt;
         double omT[RT], nxT[RT], omY[RY], nyY[RY], nxF[RY], nyF[RY], hF[RY];
+        uint32_t peer_T = 0, peer_full = 0;           // the peer's T ring and full[] barriers (shared::cluster addresses)
+        if (CL == 2) { peer_T = map_to_cta(smem_u32(Tt), peer); peer_full = map_to_cta(smem_u32(full), peer); }
 #pragma unroll
         for (int r = 0; r < RT; ++r) {
-            const int b = pt + r * NPROD;
+            const int b = pt + (r * CL + (int)my_rank) * NPROD;
             const int iw = co.bw + 4 * (b >> 6) + 2 * (b & 1) + ((b >> 4) & 1);
             const int ix = co.bx + 8 * ((b >> 5) & 1) + 2 * ((b >> 1) & 3) + ((b >> 3) & 1);
             omT[r] = P.omega[min(iw, P.n_omega - 1)];
@@ -349,7 +402,9 @@ rad_sep_kernel(const MainParams P) {
                     for (int r = 0; r < RT; ++r) {
                         const double dT = fma(-nxT[r], r89.x, fma(hxT[r], r67.y, r67.x));
                         const double2 ph = phasor_full(fma(whT[r], dT, p0T[r]));
-                        Tt[row * 256 + pt + r * NPROD] = ph;
+                        const int e = row * 256 + pt + (r * CL + (int)my_rank) * NPROD;
+                        Tt[e] = ph;
+                        if (CL == 2) st_async_v2(peer_T + (uint32_t)e * 16u, ph, peer_full + (uint32_t)buf * 8u);
                     }
 #pragma unroll
                     for (int r = 0; r < RY; ++r) {
@@ -378,7 +433,11 @@ rad_sep_kernel(const MainParams P) {
                     }
                 }
                 __syncwarp();
-                if ((pt & 31) == 0) mbar_arrive(&full[buf]);
+                if ((pt & 31) == 0) {
+                    // the peer's half of the T table arrives asynchronously: S samples x 256 / CL entries x 16 bytes
+                    if (CL == 2 && pt == 0) mbar_expect_tx(&full[buf], S * (256 / CL) * 16);
+                    else mbar_arrive(&full[buf]);
+                }
                 ++g;
                 adv = cur.step(P);
             } while (adv == 0);
@@ -387,12 +446,15 @@ rad_sep_kernel(const MainParams P) {
             producer_bar_sync<NPROD>();
             if (pt == 0) produce();
         }
+        if (CL == 2) cluster_sync_all();              // (matches the consumers' barrier at the end of the kernel)
         return;
     }
 
     // ========================================================================== CONSUMERS (phase B)
     reg_alloc<SepRegs<NC>::CONS>();
-    const SepCoord<WY> co(blockIdx.x, tid, P.n_thx, P.n_thy);
+    const SepCoord<WY> co(blockIdx.x, tid, P.n_thx, P.n_thy, CL);
+    uint32_t peer_empty = 0;
+    if (CL == 2) peer_empty = map_to_cta(smem_u32(empty), peer);
     const int64_t gid = (int64_t)blockIdx.x * SEP_CONS + tid;
     // read offsets (entries) of this thread inside one sample's tables
     const int rT = (co.ww * 2 + co.wx) * 32 + co.lx * 2 + co.lw;          // + (i*2 + j) * 8
@@ -500,7 +562,10 @@ rad_sep_kernel(const MainParams P) {
             }
         }
         __syncwarp();
-        if ((tid & 31) == 0) mbar_arrive(&empty[buf]);
+        if ((tid & 31) == 0) {
+            mbar_arrive(&empty[buf]);
+            if (CL == 2) mbar_arrive_remote(peer_empty + (uint32_t)buf * 8u);
+        }
         ++g;
         if (--todo == 0) {
             // ================================================================ end of trajectory p_now (a5, a7)
@@ -556,6 +621,7 @@ rad_sep_kernel(const MainParams P) {
             P.ang_partial[(int64_t)blockIdx.x * 16 + tid] = sum;
         }
     }
+    if (CL == 2) cluster_sync_all();                  // the peer may still store T entries / arrive here until it is done
 }
 
 // angular spectrum, second pass for the separable kernel: spec[i_w] (+)= d_solid * sum over the angle tiles of
@@ -584,7 +650,7 @@ template <int NC, int WY>
 __global__ void __launch_bounds__(SEP_CONS)
 rad_sep_finalize_kernel(const MainParams P) {
     constexpr int EV = 4 * WY;
-    const SepCoord<WY> co(blockIdx.x, threadIdx.x, P.n_thx, P.n_thy);
+    const SepCoord<WY> co(blockIdx.x, threadIdx.x, P.n_thx, P.n_thy, P.cl);
     const int64_t gid = (int64_t)blockIdx.x * SEP_CONS + threadIdx.x;
     {                                                 // gridDim.y = EV: one of the thread's points per CTA row
         const int e = blockIdx.y;
