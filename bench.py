@@ -49,11 +49,20 @@ UNIT = "evals/s"
 # 8 omegas -> 43.25 [47.6] flops, 24.6 [26.9] FP64 instructions (SURVEY.md 8(d) estimated 52-60).  Separable-phasor
 # kernel: per eval one complex multiply (6) and the accumulation (8 [12]), plus per 16 [8] evals one T and one
 # [half a] Y phasor and one [half an] integrand entry (36 + 35 + 28 [31] flops) -> 20.19 [26.63] flops, 11.75 [15.19]
-# FP64 instructions.
+# FP64 instructions.  When the separable kernel runs as cluster pairs (plan["cluster"] == 2: every BASELINE config but
+# cfg4, whose 16 x 16 angles are one tile) each CTA computes only half of the T table: 19.06 [24.38] flops, 11.09
+# [13.88] FP64 instructions per eval -- the constants below marked 'c'.
 KERNELS = {1: "rad_main_kernel (direct phasor)", 2: "rad_sep_kernel (separable phasor)",
            3: "rad_fused_kernel (single launch: pack + direct phasor + grid-wide ordered reduction)"}
-FLOPS_PER_EVAL = {1: {0: 43.25, 1: 43.25, 2: 47.6}, 2: {0: 20.19, 1: 20.19, 2: 26.63}, 3: {0: 43.25, 1: 43.25, 2: 47.6}}
-FP64_INSTR_PER_EVAL = {1: {0: 24.6, 1: 24.6, 2: 26.9}, 2: {0: 11.75, 1: 11.75, 2: 15.19}, 3: {0: 24.6, 1: 24.6, 2: 26.9}}
+FLOPS_PER_EVAL = {1: {0: 43.25, 1: 43.25, 2: 47.6}, 2: {0: 20.19, 1: 20.19, 2: 26.63}, 3: {0: 43.25, 1: 43.25, 2: 47.6},
+                  "2c": {0: 19.06, 1: 19.06, 2: 24.38}}
+FP64_INSTR_PER_EVAL = {1: {0: 24.6, 1: 24.6, 2: 26.9}, 2: {0: 11.75, 1: 11.75, 2: 15.19}, 3: {0: 24.6, 1: 24.6, 2: 26.9},
+                       "2c": {0: 11.09, 1: 11.09, 2: 13.88}}
+
+
+def work_key(plan):
+    """Key into the two tables above for the kernel of a plan's first part."""
+    return "2c" if plan["kernel"] == 2 and plan.get("cluster", 1) == 2 else plan["kernel"]
 FP64_SPEC_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # 148 SM x 64 FMA lanes x 2 x 1.965 GHz
 MODELS = ["classical", "spin0", "spin1/2"]
 # dram__bytes_read.sum + dram__bytes_write.sum per main-kernel launch from the committed ncu --set full captures
@@ -331,14 +340,16 @@ class Bench:
         if not r["main_ms"] or evals == 0:
             return None
         main_s = float(np.mean(r["main_ms"])) * 1e-3
-        k = plan["kernel"]
+        k, wk = plan["kernel"], work_key(plan)
         if plan["parts"] == 2:                                         # separable interior + direct rest
             frac_sep = plan["interior_x"] * plan["interior_y"] / (len(wl.thx) * len(wl.thy))
-            flops = evals * (frac_sep * FLOPS_PER_EVAL[2][model] + (1 - frac_sep) * FLOPS_PER_EVAL[1][model])
-            instr = evals * (frac_sep * FP64_INSTR_PER_EVAL[2][model] + (1 - frac_sep) * FP64_INSTR_PER_EVAL[1][model])
+            flops = evals * (frac_sep * FLOPS_PER_EVAL[wk][model] + (1 - frac_sep) * FLOPS_PER_EVAL[1][model])
+            instr = evals * (frac_sep * FP64_INSTR_PER_EVAL[wk][model] + (1 - frac_sep) * FP64_INSTR_PER_EVAL[1][model])
             name = f"{KERNELS[2]} on {plan['interior_x']} x {plan['interior_y']} angles + {KERNELS[1]} on the rest"
         else:
-            flops, instr, name = evals * FLOPS_PER_EVAL[k][model], evals * FP64_INSTR_PER_EVAL[k][model], KERNELS[k]
+            flops, instr, name = evals * FLOPS_PER_EVAL[wk][model], evals * FP64_INSTR_PER_EVAL[wk][model], KERNELS[k]
+        if wk == "2c":
+            name += ", cluster pairs sharing the T table"
         achieved = flops / main_s
         key = f"{wl.name}|{k}"
         return {"bound": "alu", "kernel": name, "achieved": achieved / 1e12, "peak": self.peak / 1e12, "unit": "TFLOP/s",

@@ -489,9 +489,10 @@ def rad_plan_kernel(n_omega: int, n_thx: int, n_thy: int, model: int = CLASSICAL
 def rad_plan_describe(count: int, n_max: int, n_omega: int, n_thx: int, n_thy: int, model: int = CLASSICAL,
                       kernel: int = 0) -> dict:
     """Launch plan of a call of this shape (include/rad.h rad_plan_describe)."""
-    plan = (ctypes.c_int32 * 10)()
+    plan = (ctypes.c_int32 * 11)()
     _check(load_library().rad_plan_describe(count, n_max, n_omega, n_thx, n_thy, int(model), int(kernel), plan))
-    keys = ("kernel", "mode", "tiles", "slices", "t_slices", "chunks", "parts", "interior_x", "interior_y", "launches")
+    keys = ("kernel", "mode", "tiles", "slices", "t_slices", "chunks", "parts", "interior_x", "interior_y", "launches",
+            "cluster")
     return dict(zip(keys, (int(v) for v in plan)))
 
 

@@ -807,13 +807,7 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const int64
         mp.partial = reinterpret_cast<double *>(ws + pt.off_partial);
         mp.t_pad = pl.t_pad;
         mp.l_x0 = pt.l_x0; mp.l_y0 = pt.l_y0;
-        mp.cl = 1;
-#ifndef RAD_SEP_NO_CLUSTER
-        if (pt.kernel == K_SEP) {                     // an even number of y tiles: cluster pairs share the T table
-            const int ty = nc == 6 ? 8 : 16;
-            if (((pt.n_thy + ty - 1) / ty) % 2 == 0) mp.cl = 2;
-        }
-#endif
+        mp.cl = pt.cl;
         if (ang) {
             mp.ang = 1; mp.cut2 = ang->cut2;
             mp.ang_groups = std::min((g->n_omega + W - 1) / W, (TPB + pt.angles - 1) / pt.angles + 1);
@@ -1178,6 +1172,7 @@ int rad_plan_describe(int32_t count, int64_t n_max, int32_t n_omega, int32_t n_t
     plan[7] = !cp.fused && cp.nparts == 2 ? cp.part[0].n_thx : 0;
     plan[8] = !cp.fused && cp.nparts == 2 ? cp.part[0].n_thy : 0;
     plan[9] = cp.launches();
+    plan[10] = cp.fused ? 1 : cp.part[0].cl;
     return RAD_OK;
 }
 

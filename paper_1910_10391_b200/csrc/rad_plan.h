@@ -43,6 +43,8 @@ struct Part {
     int angles;               // angles the part evaluates
     Plan plan;
     size_t off_partial;
+    int cl;                   // separable kernel: 2 = launched as cluster pairs of CTAs on neighbouring y tiles that
+                              // share the T table through distributed shared memory (needs an even y tile count)
 };
 
 struct CallPlan {
@@ -123,7 +125,7 @@ static inline void choose_parts(int n_omega, int n_thx, int n_thy, int nc, int k
                                 Part *part, int &nparts) {
     const int ty = nc == 6 ? 8 : 16;
     auto whole = [&](int k) {
-        part[0] = Part{k, n_thx, n_thy, -1, -1, n_thx * n_thy, Plan{}, 0};
+        part[0] = Part{k, n_thx, n_thy, -1, -1, n_thx * n_thy, Plan{}, 0, 1};
         nparts = 1;
     };
     if (kernel == 1) return whole(K_DIRECT);
@@ -149,8 +151,8 @@ static inline void choose_parts(int n_omega, int n_thx, int n_thy, int nc, int k
             }
     }
     if (bx > 0) {
-        part[0] = Part{K_SEP, bx, by, -1, -1, bx * by, Plan{}, 0};
-        part[1] = Part{K_DIRECT, n_thx, n_thy, bx, by, n_thx * n_thy - bx * by, Plan{}, 0};
+        part[0] = Part{K_SEP, bx, by, -1, -1, bx * by, Plan{}, 0, 1};
+        part[1] = Part{K_DIRECT, n_thx, n_thy, bx, by, n_thx * n_thy - bx * by, Plan{}, 0, 1};
         nparts = 2;
         return;
     }
@@ -206,6 +208,13 @@ static inline CallPlan plan_call(int count, int64_t n_max, int n_omega, int n_th
                                         : split_plan(K_SEP, count, cp.cpt, n_omega, pt.n_thx, pt.n_thy, nc, sms);
         pt.off_partial = off;
         off += pt.plan.partial_bytes;
+        pt.cl = 1;
+#ifndef RAD_SEP_NO_CLUSTER
+        if (pt.kernel == K_SEP) {
+            const int ty = nc == 6 ? 8 : 16;
+            if (((pt.n_thy + ty - 1) / ty) % 2 == 0) pt.cl = 2;
+        }
+#endif
     }
     if (cp.fused) {           // partial amplitudes of the fused kernel: [slices][nc * W][tiles * FUSED_TPB]
         cp.part[0].off_partial = cp.off_packed;       // it needs no packed buffer: reuse the space from the start

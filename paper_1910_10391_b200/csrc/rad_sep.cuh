@@ -32,7 +32,7 @@ constexpr int SEP_CONS = 256;  // consumer threads
 #define RAD_SEP_PROD4 128
 #endif
 #ifndef RAD_SEP_PROD6
-#define RAD_SEP_PROD6 128
+#define RAD_SEP_PROD6 256
 #endif
 #ifndef RAD_SEP_S
 #define RAD_SEP_S 8
@@ -47,13 +47,19 @@ constexpr int SEP_CONS = 256;  // consumer threads
 #define RAD_SEP_REGS_CONS4 192
 #endif
 #ifndef RAD_SEP_REGS_CONS6
-#define RAD_SEP_REGS_CONS6 176
+#define RAD_SEP_REGS_CONS6 168
 #endif
 #ifndef RAD_SEP_PU4
 #define RAD_SEP_PU4 1
 #endif
 #ifndef RAD_SEP_PU6
-#define RAD_SEP_PU6 8
+#define RAD_SEP_PU6 4
+#endif
+#ifndef RAD_SEP_HS4                 // sample groups of the producers: NPROD / HS threads own the table entries, group h
+#define RAD_SEP_HS4 1               // of them fills samples [h S / HS, (h + 1) S / HS) of every sub-block
+#endif
+#ifndef RAD_SEP_HS6
+#define RAD_SEP_HS6 2
 #endif
 constexpr int SEP_S = RAD_SEP_S;       // samples per table sub-block
 constexpr int SEP_NB = RAD_SEP_NB;     // table buffers in flight
@@ -61,13 +67,20 @@ constexpr int SEP_STAGES = 3;  // trajectory-chunk ring depth
 // Producer threads per CTA (RAD_SEP_PROD4 / RAD_SEP_PROD6) and the register split.
 // setmaxnreg moves registers between the roles inside the pool the CTA got at launch
 // (THREADS * REGS_LAUNCH): 256 * CONS + NPROD * PROD <= that pool, both multiples of 8.
-// Measured (round 2, ncu source page): with 6 accumulators per point the tables serve only 8 points per
-// consumer thread and the kernel is PRODUCER-bound -- the four producer warps never wait, the consumers
-// wait for tables 17-21 % of their time.  What helped: unrolling the producers' sample loop fully
-// (RAD_SEP_PU6 = 8: 32 independent phasor chains per thread instead of 4) and moving registers to them
-// (176 / 152 instead of 200 / 104): +5.8 %.  What did not: eight producer warps with one T and one Y-or-F
-// entry per thread (RAD_SEP_PROD6 = 256, 80-96 registers each: spills, -3 ... -10 %), finer or deeper table
-// rings (4-sample sub-blocks x 4), the magic-number range reduction instead of FRND.F64 (+-0).
+// Measured (round 2, ncu source page split by role): with 6 accumulators per point the tables serve only 8 points
+// per consumer thread and the kernel is PRODUCER-bound: the consumers wait for tables 14-21 % of their time while a
+// lone producer warp per sub-partition issues only 13-15 % of the cycles -- it is latency-bound (fixed-latency
+// dependency 31 %, shared-memory scoreboard 18 %), not short of issue slots.  Steps, each measured on config 3:
+//   * full unroll of the producers' sample loop + registers moved to them (176 / 152)              +5.8 %
+//   * cluster pairs sharing the T table (-25 % producer work; see rad_sep_kernel)                   +5.9 %
+//   * EIGHT producer warps as two sample groups (RAD_SEP_HS6 = 2: threads [0, 128) fill samples 0-3 of a
+//     sub-block, threads [128, 256) samples 4-7, same entries), 168 / 88 registers, 4-sample unroll   +7.0 %
+//     (two warps per sub-partition overlap each other's latencies; 160 / 96: -0.7 %, 152 / 104: -7 %: the
+//     consumers' 48 accumulators + 20 table entries in flight need their 168)
+// With 4 accumulators per point (classical, spin-0) the consumers wait only 4 % and need 192 registers: eight
+// producer warps (184 / 72, 176 / 80) lose 4-10 % there, so that variant keeps four.
+// What did not help: one T and one Y-or-F entry per thread for eight producer warps (round 1), finer or deeper
+// table rings (4-sample sub-blocks x 4), the magic-number range reduction instead of FRND.F64 (+-0).
 template <int NC> struct SepRegs {
     static constexpr int NPROD = NC == 6 ? RAD_SEP_PROD6 : RAD_SEP_PROD4;     // producer threads
     static constexpr int THREADS = SEP_CONS + NPROD;
@@ -77,6 +90,9 @@ template <int NC> struct SepRegs {
     // samples the producers work on at once: their phasor chains are ~15 dependent FP64 steps long, and one
     // producer warp per sub-partition has only its own instruction-level parallelism to hide that latency
     static constexpr int PROD_UNROLL = NC == 6 ? RAD_SEP_PU6 : RAD_SEP_PU4;
+    static constexpr int HS = NC == 6 ? RAD_SEP_HS6 : RAD_SEP_HS4;            // sample groups
+    static constexpr int NE = NPROD / HS;                                     // threads that own table entries
+    static_assert(NPROD % HS == 0 && NE % 32 == 0 && SEP_S % HS == 0, "sample groups are whole warps");
     static_assert(CONS % 8 == 0 && PROD >= 24 && SEP_CONS * CONS + NPROD * PROD <= THREADS * REGS_LAUNCH,
                   "setmaxnreg.inc would wait forever for registers the CTA does not own");
 };
@@ -299,19 +315,20 @@ rad_sep_kernel(const MainParams P) {
         // Entries per thread and sample.  T: 256 / NPROD.  Y and F: YN / NPROD each, or -- when there are more
         // producer threads than Y entries -- one Y entry for threads [0, YN) and one F entry for the rest
         // (whole warps take one role: YN is a multiple of 32).
-        constexpr int NPROD = SepRegs<NC>::NPROD;
-        constexpr bool SPLIT = YN < NPROD;
-        static_assert(256 % NPROD == 0 && (SPLIT ? 2 * YN == NPROD : YN % NPROD == 0), "producer entry assignment");
-        static_assert((256 / NPROD) % CL == 0, "the T entries of a thread are dealt out to the CTAs of the pair");
-        constexpr int RT = 256 / NPROD / CL, RY = SPLIT ? 1 : YN / NPROD;   // CL = 2: entry slots r * CL + rank
-        const bool doY = !SPLIT || pt < YN, doF = !SPLIT || pt >= YN;
-        const int ptF = SPLIT ? (pt >= YN ? pt - YN : 0) : pt, ptY = SPLIT ? (pt < YN ? pt : 0) : pt;
+        constexpr int NPROD = SepRegs<NC>::NPROD, NE = SepRegs<NC>::NE, HS = SepRegs<NC>::HS;
+        const int pe = pt % NE, hs = pt / NE;            // entry slot, sample group
+        constexpr bool SPLIT = YN < NE;
+        static_assert(256 % NE == 0 && (SPLIT ? 2 * YN == NE : YN % NE == 0), "producer entry assignment");
+        static_assert((256 / NE) % CL == 0, "the T entries of a thread are dealt out to the CTAs of the pair");
+        constexpr int RT = 256 / NE / CL, RY = SPLIT ? 1 : YN / NE;         // CL = 2: entry slots r * CL + rank
+        const bool doY = !SPLIT || pe < YN, doF = !SPLIT || pe >= YN;
+        const int ptF = SPLIT ? (pe >= YN ? pe - YN : 0) : pe, ptY = SPLIT ? (pe < YN ? pe : 0) : pe;
         double omT[RT], nxT[RT], omY[RY], nyY[RY], nxF[RY], nyF[RY], hF[RY];
         uint32_t peer_T = 0, peer_full = 0;           // the peer's T ring and full[] barriers (shared::cluster addresses)
         if (CL == 2) { peer_T = map_to_cta(smem_u32(Tt), peer); peer_full = map_to_cta(smem_u32(full), peer); }
 #pragma unroll
         for (int r = 0; r < RT; ++r) {
-            const int b = pt + (r * CL + (int)my_rank) * NPROD;
+            const int b = pe + (r * CL + (int)my_rank) * NE;
             const int iw = co.bw + 4 * (b >> 6) + 2 * (b & 1) + ((b >> 4) & 1);
             const int ix = co.bx + 8 * ((b >> 5) & 1) + 2 * ((b >> 1) & 3) + ((b >> 3) & 1);
             omT[r] = P.omega[min(iw, P.n_omega - 1)];
@@ -320,7 +337,7 @@ rad_sep_kernel(const MainParams P) {
 #pragma unroll
         for (int r = 0; r < RY; ++r) {
             {
-                const int b = ptY + r * NPROD;
+                const int b = ptY + r * NE;
                 const int q = b >> 3, m = q % WY, i = (q / WY) & 1, ww = (q / WY) >> 1;
                 const int iw = co.bw + 4 * ww + 2 * (b & 1) + i;
                 const int iy = co.by + WY * ((b >> 1) & 3) + m;
@@ -328,7 +345,7 @@ rad_sep_kernel(const MainParams P) {
                 nyY[r] = P.thy[min(iy, P.n_thy - 1)];
             }
             {
-                const int b = ptF + r * NPROD;
+                const int b = ptF + r * NE;
                 const int q = b >> 4, m = q % WY, j = (q / WY) & 1, wx = (q / WY) >> 1;
                 const int ix = co.bx + 8 * wx + 2 * ((b >> 2) & 3) + j;
                 const int iy = co.by + WY * (b & 3) + m;
@@ -392,17 +409,17 @@ rad_sep_kernel(const MainParams P) {
             do {                                         // sub-blocks of this chunk
                 const int buf = g % NB;
                 mbar_wait(&empty[buf], ((g / NB) & 1) ^ 1);
-                const double *rec = ck + HDR + cur.sb * S * REC;
+                const double *rec = ck + HDR + (cur.sb * S + hs * (S / HS)) * REC;
 #pragma unroll SepRegs<NC>::PROD_UNROLL
-                for (int s = 0; s < S; ++s, rec += REC) {
-                    const int row = buf * S + s;
+                for (int s0 = 0; s0 < S / HS; ++s0, rec += REC) {
+                    const int row = buf * S + hs * (S / HS) + s0;
                     const double2 r67 = *reinterpret_cast<const double2 *>(rec + 6);   // dP0, dt
                     const double2 r89 = *reinterpret_cast<const double2 *>(rec + 8);   // dx, dy
 #pragma unroll
                     for (int r = 0; r < RT; ++r) {
                         const double dT = fma(-nxT[r], r89.x, fma(hxT[r], r67.y, r67.x));
                         const double2 ph = phasor_full(fma(whT[r], dT, p0T[r]));
-                        const int e = row * 256 + pt + (r * CL + (int)my_rank) * NPROD;
+                        const int e = row * 256 + pe + (r * CL + (int)my_rank) * NE;
                         Tt[e] = ph;
                         if (CL == 2) st_async_v2(peer_T + (uint32_t)e * 16u, ph, peer_full + (uint32_t)buf * 8u);
                     }
@@ -411,7 +428,7 @@ rad_sep_kernel(const MainParams P) {
                         if (!doY) continue;
                         const double dY = fma(-nyY[r], r89.y, hyY[r] * r67.y);
                         const double2 ph = phasor_full(fma(whY[r], dY, p0Y[r]));
-                        Yt[row * YN + ptY + r * NPROD] = ph;
+                        Yt[row * YN + ptY + r * NE] = ph;
                     }
                     if (!doF) continue;
                     const double2 r01 = *reinterpret_cast<const double2 *>(rec);       // D0, vx
@@ -427,9 +444,9 @@ rad_sep_kernel(const MainParams P) {
                         const double gq = inv_square(q);
                         const double s1 = fma(nyF[r], r45.x, r45.y);
                         const double s2 = fma(nxF[r], r23.y, r45.y);
-                        Ft[row * YN + ptF + r * NPROD] = make_double2(fma(s1, ux, -(bx * r23.y)) * gq,
+                        Ft[row * YN + ptF + r * NE] = make_double2(fma(s1, ux, -(bx * r23.y)) * gq,
                                                                       fma(s2, uy, -(by * r45.x)) * gq);
-                        if (NC == 6) Hh[row * YN + ptF + r * NPROD] = fma(nxF[r], r23.y, s1) * gq;
+                        if (NC == 6) Hh[row * YN + ptF + r * NE] = fma(nxF[r], r23.y, s1) * gq;
                     }
                 }
                 __syncwarp();

@@ -58,8 +58,9 @@ def test_flop_constants_are_consistent_with_the_issue_rate(rad, kernel, model):
     t = float(np.median(ms)) * 1e-3
     plan = rad.rad_plan_describe(1, len(wl.traj["t"]), len(wl.omega), len(wl.thx), len(wl.thy), model, kernel)
     assert plan["kernel"] == kernel and plan["parts"] == 1
-    frac = bench.FLOPS_PER_EVAL[kernel][model] * wl.evals / t / peak
-    issue = bench.FP64_INSTR_PER_EVAL[kernel][model] * wl.evals / t / (peak / 2)
+    wk = bench.work_key(plan)                                          # "2c": separable kernel as cluster pairs
+    frac = bench.FLOPS_PER_EVAL[wk][model] * wl.evals / t / peak
+    issue = bench.FP64_INSTR_PER_EVAL[wk][model] * wl.evals / t / (peak / 2)
     assert frac <= issue <= 1.0, (frac, issue)
     assert frac >= (0.2 if kernel == 3 else 0.45), frac               # cfg1 is a 30 us problem: launch + tail dominate
     assert 0.9 * bench.FP64_SPEC_TFLOPS <= peak / 1e12 <= 1.05 * bench.FP64_SPEC_TFLOPS
