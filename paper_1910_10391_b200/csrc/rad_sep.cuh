@@ -225,34 +225,37 @@ template <int NPROD> __device__ __forceinline__ void producer_bar_sync() {   // 
 // their own copy: both sides derive the same sequence from the launch parameters, so the only thing
 // they exchange is table buffers.
 struct SepCursor {
+    static constexpr int SPC = CH / SEP_S;   // sub-blocks per chunk
     int p, p_end, ts;
     int c, c1;                 // chunk index, end of this trajectory's chunk range
-    int sb, nsb;               // sub-block inside the chunk, sub-blocks of this chunk
+    int sb, nsb;               // sub-block inside the chunk, end of this slice's sub-blocks inside the chunk
+    int s_end;                 // end of the slice's sub-block range (index inside the trajectory)
     __device__ __forceinline__ SepCursor(const MainParams &P, int slice) {
         ts = 0;
         if (P.mode == MODE_TSPLIT) { p = slice / P.t_slices; p_end = p + 1; ts = slice % P.t_slices; }
         else { p = (int)((int64_t)slice * P.count / P.p_slices);
                p_end = (int)((int64_t)(slice + 1) * P.count / P.p_slices); }
-        sb = 0; nsb = 0; c = 0; c1 = 0;
+        sb = 0; nsb = 0; c = 0; c1 = 0; s_end = 0;
         seek(P);
     }
     static __device__ __forceinline__ int64_t n_of(const MainParams &P, int q) {
         return P.n_dev ? P.n_dev[q] : P.n_single;
     }
-    __device__ __forceinline__ void chunk_range(const MainParams &P, int q, int &c0, int &cend) const {
-        const int nch = (int)((n_of(P, q) + CH - 1) / CH);
-        if (P.mode == MODE_TSPLIT) { c0 = (int)((int64_t)ts * nch / P.t_slices);
-                                     cend = (int)((int64_t)(ts + 1) * nch / P.t_slices); }
-        else { c0 = 0; cend = nch; }
+    // Sub-blocks [s0, s1) of trajectory q that belong to this slice.  A time slice is a range of SUB-BLOCKS (8
+    // samples), not of chunks: 24 chunks over 7 slices would give some CTAs 4 chunks and others 3 (the paper's
+    // typical grid with N = 3000); 375 sub-blocks over 7 slices differ by one in 54.
+    __device__ __forceinline__ void sb_range(const MainParams &P, int q, int &s0, int &s1) const {
+        const int nsbt = (int)((n_of(P, q) + SEP_S - 1) / SEP_S);
+        if (P.mode == MODE_TSPLIT) { s0 = (int)((int64_t)ts * nsbt / P.t_slices);
+                                     s1 = (int)((int64_t)(ts + 1) * nsbt / P.t_slices); }
+        else { s0 = 0; s1 = nsbt; }
     }
-    __device__ __forceinline__ void set_nsb(const MainParams &P) {
-        const int64_t left = n_of(P, p) - (int64_t)c * CH;
-        nsb = ((int)min((int64_t)CH, left) + SEP_S - 1) / SEP_S;
-    }
-    __device__ __forceinline__ void seek(const MainParams &P) {   // first trajectory from p on with chunks to do
+    __device__ __forceinline__ void set_nsb() { nsb = min(SPC, s_end - c * SPC); }
+    __device__ __forceinline__ void seek(const MainParams &P) {   // first trajectory from p on with sub-blocks to do
         while (p < p_end) {
-            chunk_range(P, p, c, c1);
-            if (c < c1) { set_nsb(P); break; }
+            int s0, s1;
+            sb_range(P, p, s0, s1);
+            if (s0 < s1) { c = s0 / SPC; c1 = (s1 + SPC - 1) / SPC; sb = s0 % SPC; s_end = s1; set_nsb(); break; }
             ++p;
         }
     }
@@ -261,7 +264,7 @@ struct SepCursor {
     __device__ __forceinline__ int step(const MainParams &P) {
         if (++sb < nsb) return 0;
         sb = 0;
-        if (++c < c1) { set_nsb(P); return 1; }
+        if (++c < c1) { set_nsb(); return 1; }
         ++p;
         seek(P);
         return 2;
@@ -511,18 +514,20 @@ rad_sep_kernel(const MainParams P) {
     int p_now = cur.p;
     const int p_end = cur.p_end;
     auto sub_blocks_of = [&](int p) -> int {          // sub-blocks of trajectory p inside this slice
-        int c0, c1;
-        cur.chunk_range(P, p, c0, c1);
-        if (c0 >= c1) return 0;
-        const int64_t left = SepCursor::n_of(P, p) - (int64_t)(c1 - 1) * CH;      // samples of the last chunk
-        return (c1 - 1 - c0) * (CH / S) + ((int)min((int64_t)CH, left) + S - 1) / S;
+        int s0, s1;
+        cur.sb_range(P, p, s0, s1);
+        return s1 - s0;
     };
     int todo = p_now < p_end ? sub_blocks_of(p_now) : 0;
     uint32_t g = 0;
     while (p_now < p_end) {
         const int buf = g % NB;
         mbar_wait(&full[buf], (g / NB) & 1);
-#pragma unroll
+#ifndef RAD_SEP_CU
+#define RAD_SEP_CU 8
+#endif
+        constexpr int CU = RAD_SEP_CU;
+#pragma unroll CU
         for (int s = 0; s < S; ++s) {                 // a4: complex multiply + accumulate
             const int row = buf * S + s;
             const double2 *tp = Tt + row * 256 + rT, *yp = Yt + row * YN + rY, *fp = Ft + row * YN + rF;
@@ -549,12 +554,17 @@ rad_sep_kernel(const MainParams P) {
                     pi[i] = fma(tv[i][j].y, y.x, pi[i]);
                 }
             };
-            products(0, qr, qi);
+            // (The 64 accumulators of the 4-per-point variant leave ptxas so few registers that it renames
+            // accumulators and moves them back: 106-194 IMAD.MOV per 1007 FP64 instructions of the loop, depending on
+            // unrelated code around it; staged or not changes the throughput by +-1 %.)
+            constexpr bool STAGED = true;
+            if (STAGED) products(0, qr, qi);
 #pragma unroll
             for (int g = 0; g < G; ++g) {
                 const int m = g >> 1, j = g & 1;
                 double nr[2], ni[2];
-                if (g + 1 < G) products(g + 1, nr, ni);
+                if (!STAGED) products(g, qr, qi);
+                else if (g + 1 < G) products(g + 1, nr, ni);
                 const double2 f = fp[(j * WY + m) * 16];
                 double *a0 = acc[(0 * 2 + j) * WY + m], *a1 = acc[(1 * 2 + j) * WY + m];
                 a0[0] = fma(f.x, qr[0], a0[0]);
@@ -572,7 +582,7 @@ rad_sep_kernel(const MainParams P) {
                     a1[4] = fma(hv, qr[1], a1[4]);
                     a1[5] = fma(hv, qi[1], a1[5]);
                 }
-                if (g + 1 < G) {
+                if (STAGED && g + 1 < G) {
 #pragma unroll
                     for (int i = 0; i < 2; ++i) { qr[i] = nr[i]; qi[i] = ni[i]; }
                 }
