@@ -66,8 +66,22 @@ def work_key(plan):
 FP64_SPEC_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # 148 SM x 64 FMA lanes x 2 x 1.965 GHz
 MODELS = ["classical", "spin0", "spin1/2"]
 # dram__bytes_read.sum + dram__bytes_write.sum per main-kernel launch from the committed ncu --set full captures
-# (bench.py cannot run ncu itself): profiles/r02_ncu_traffic.json, written next to the captures it summarises.
-TRAFFIC_FILE = ROOT / "profiles" / "r02_ncu_traffic.json"
+# (bench.py cannot run ncu itself): profiles/r02_ncu_traffic.csv (workload, kernel code, bytes, capture file), written
+# next to the captures it summarises.
+TRAFFIC_FILE = ROOT / "profiles" / "r02_ncu_traffic.csv"
+
+
+def read_traffic(path=TRAFFIC_FILE):
+    """{"<workload name>|<kernel code>": dram bytes per main-kernel launch} from the committed table; {} if absent."""
+    table = {}
+    try:
+        for ln in Path(path).read_text().splitlines():
+            f = [x.strip() for x in ln.split(",")]
+            if len(f) >= 3 and f[0] and not f[0].startswith("#") and f[0] != "workload":
+                table[f"{f[0]}|{f[1]}"] = float(f[2])
+    except OSError:
+        pass
+    return table
 
 
 def parse():
@@ -243,10 +257,7 @@ class Bench:
         self.flush = torch.empty(256 << 20, dtype=torch.uint8, device=self.dev)      # > 126 MB L2
         self.peak = rad.rad_measure_fp64_peak(300.0)                                 # FLOP/s, measured here
         self.prof = rad.RadProfile()
-        try:
-            self.traffic = json.loads(TRAFFIC_FILE.read_text())
-        except Exception:
-            self.traffic = {}
+        self.traffic = read_traffic()
 
     def barrier(self):
         if self.world > 1:
@@ -411,6 +422,46 @@ class Bench:
         return wl.evals * steps / wall, h2d, host_out.numel() * 8, steps
 
 
+def generator_throughput(B):
+    """rad_generate_trajectories on its own -- 2000 particles (the paper's ensembles: up to
+    2000 particles) x 20 000 steps in each of the three synthetic wells, device time by CUDA events.
+    One thread per particle and a serial recurrence per step: the bound is the latency of that dependent chain, not
+    HBM; the HBM figure (88 B written per particle and step against the measured copy bandwidth) is reported so that
+    this is visible."""
+    import math
+    torch, rad = B.torch, B.rad
+    try:
+        hbm = json.loads((ROOT / "MEASURED_PEAKS.json").read_text())["hbm_gbs"] * 1e9
+        hbm_kind = "measured (MEASURED_PEAKS.json)"
+    except Exception:
+        hbm, hbm_kind = 6.65e12, "fallback (B200_PROFILING.md)"
+    wells = {"cosine (cfg3)": (0, math.pi * 5e-5 ** 2 / (2 * 1.92e-10), 1.92e-10, 39139.0, 1e-9, 0.0),
+             "axial exp (cfg5)": (1, 3e-5 ** 2 / (2 * 0.3e-10), 0.3e-10, 97847.0, 1e-9, 0.0),
+             "harmonic + kicks (cfg2/4)": (2, (2 * math.pi / 7e-6) ** 2, 1.0, 9784.7, 7e-9, 2e-7)}
+    count, n = 2000, 20000
+    rng = np.random.Generator(np.random.PCG64(99))
+    ini = [B.to_dev(a) for a in (rng.uniform(-4e-11, 4e-11, count), rng.uniform(-4e-11, 4e-11, count),
+                                 rng.uniform(-1e-5, 1e-5, count), rng.uniform(-1e-5, 1e-5, count))]
+    out = {k: torch.empty((count, n), dtype=torch.float64, device=B.dev) for k in rad.FIELDS}
+    res = {}
+    for name, (well, kappa, length, gamma, dt, sigma) in wells.items():
+        def call():
+            rad.rad_generate_trajectories(well, kappa, length, gamma, dt, n, *ini, out=out, sigma=sigma, seed=7)
+        for _ in range(2):
+            call()
+        a, b = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        a.record()
+        for _ in range(3):
+            call()
+        b.record()
+        torch.cuda.synchronize()
+        sec = a.elapsed_time(b) * 1e-3 / 3
+        res[name] = {"particle_steps_per_s": count * n / sec, "ms": sec * 1e3, "bytes_written_per_s": 88.0 * count * n / sec,
+                     "frac_of_hbm": 88.0 * count * n / sec / hbm}
+    return {"particles": count, "steps": n, "hbm_peak_kind": hbm_kind, "bound": "latency of the per-particle recurrence",
+            "wells": res}
+
+
 def run_b200(args):
     B = Bench(args)
     world, rank = B.world, B.rank
@@ -485,6 +536,8 @@ def run_b200(args):
             line["rank_ms_per_step"] = head["rank_ms_per_step"]
         if per_config:
             line["per_config"] = per_config
+            if world == 1:
+                line["trajectory_generator"] = generator_throughput(B)
         if not args.no_cpu_baseline and world == 1:
             line["cpu_baseline"] = cpu_baseline(wl)
         print(json.dumps(line))

@@ -84,18 +84,18 @@ def test_bench_line_contract_on_a_small_workload():
 
 
 def test_traffic_table_names_kernels_that_exist():
-    """profiles/r02_ncu_traffic.json (dram bytes per main-kernel launch from the committed ncu captures) is keyed by
-    "<workload name>|<kernel code>"; every key must name a workload bench.py can build."""
-    f = ROOT / "profiles" / "r02_ncu_traffic.json"
-    if not f.exists():
+    """profiles/r02_ncu_traffic.csv (dram bytes per main-kernel launch from the committed ncu captures) is keyed by
+    workload name and kernel code; every row must name a workload bench.py can build."""
+    import bench
+    if not bench.TRAFFIC_FILE.exists():
         pytest.skip("no traffic table committed yet")
     names = {workloads.make(n, **kw).name for n, kw in (("cfg1", {}), ("cfg2", {}), ("paper_typical", {}),
                                                        ("cfg3", dict(n=10, n_omega=1, n_th=1)),
                                                        ("cfg5", dict(n=10, n_omega=1, n_th=1)),
                                                        ("cfg5", dict(n=10, n_omega=1, n_th=1, model=1)),
                                                        ("cfg4", dict(count=1, n=10, n_omega=1, n_th=1)))}
-    for key, val in json.loads(f.read_text()).items():
-        if key.startswith("_"):
-            continue
+    table = bench.read_traffic()
+    assert table
+    for key, val in table.items():
         name, code = key.split("|")
         assert name in names and code in ("1", "2", "3") and val > 0

@@ -434,6 +434,44 @@ def test_sep_ensembles(sep_kernel, oracle_mod, model):
     assert_parity(both, ref, label=f"sep ensemble accumulate model {model}")
 
 
+def test_sep_cluster_pairs_time_and_trajectory_split(sep_kernel, oracle_mod):
+    """The separable kernel as thread-block cluster pairs (an even number of theta_y tiles: the two CTAs of a pair
+    share their T table through distributed shared memory) in the two split modes the full-size
+    configs do not reach with ragged input: a time split of one short trajectory (classical, 2 y tiles of 16) and a
+    trajectory split of a ragged ensemble with empty-ish members (spin-1/2, 2 y tiles of 8); an odd tile count next
+    to it runs as single CTAs.  Bit-identical from run to run."""
+    import torch
+    rad = sep_kernel
+    wl = workloads.make("cfg2", n=1500, n_omega=20, n_th=20, seed=31)
+    thx = wl.thx[:5].copy()
+    g = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (wl.omega, thx, wl.thy)]
+    plan = rad.rad_plan_describe(1, 1500, 20, 5, 20, CL, 2)
+    assert plan["cluster"] == 2 and plan["mode"] == 2 and plan["kernel"] == 2
+    tr = dev_dict(wl.traj)
+    cube = rad.rad_classical(tr, *g)
+    again = rad.rad_classical(tr, *g)
+    assert torch.equal(cube, again)
+    w, nx, ny = oracle_mod.grid_points(wl.omega, thx, wl.thy)
+    assert_parity(cube.cpu().numpy(), oracle_mod.points(wl.traj, w, nx, ny, CL, 0.0), label="cluster time split")
+    assert rad.rad_plan_describe(1, 1500, 20, 5, 40, CL, 2)["cluster"] == 1        # 3 y tiles: single CTAs
+
+    we = workloads.make("cfg4", count=40, n=260, n_omega=9, n_th=11, seed0=1234)
+    thx = we.thx[:6].copy()
+    rng = np.random.Generator(np.random.PCG64(5))
+    nvec = rng.integers(2, 261, size=40).astype(np.int64)
+    nvec[[0, 7, 39]] = 2
+    lam = np.linspace(0.1, 0.6, 40) / we.omega.max()
+    plan = rad.rad_plan_describe(40, 260, 9, 6, 11, SH, 2)
+    assert plan["cluster"] == 2 and plan["mode"] == 1
+    ge = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (we.omega, thx, we.thy)]
+    b = dev_dict(we.batch)
+    cube = rad.rad_ensemble_sum(b, nvec, *ge, model=SH, hbarc_over_E=lam)
+    assert torch.equal(cube, rad.rad_ensemble_sum(b, nvec, *ge, model=SH, hbarc_over_E=lam))
+    w, nx, ny = oracle_mod.grid_points(we.omega, thx, we.thy)
+    assert_parity(cube.cpu().numpy(), oracle_mod.ensemble_points(we.batch, nvec, w, nx, ny, SH, lam),
+                  label="cluster trajectory split")
+
+
 # ------------------------------------------------------------------ edge cases through the separable kernel too
 def test_sep_straight_line_domain_and_workspace(sep_kernel, oracle_mod):
     """P1 (zero acceleration -> exactly 0), u >= 1 -> NaN only there, caller workspace == pool scratch,
