@@ -51,18 +51,21 @@ UNIT = "evals/s"
 # [half a] Y phasor and one [half an] integrand entry (36 + 35 + 28 [31] flops) -> 20.19 [26.63] flops, 11.75 [15.19]
 # FP64 instructions.  When the separable kernel runs as cluster pairs (plan["cluster"] == 2: every BASELINE config but
 # cfg4, whose 16 x 16 angles are one tile) each CTA computes only half of the T table: 19.06 [24.38] flops, 11.09
-# [13.88] FP64 instructions per eval -- the constants below marked 'c'.
+# [13.88] FP64 instructions per eval -- the constants below marked '2c'.  cfg4's single angle tile pairs along omega
+# instead and halves the F table (plan["cluster"] == 3, classical only): 19.31 flops, 11.19 instructions -- '2w'.
 KERNELS = {1: "rad_main_kernel (direct phasor)", 2: "rad_sep_kernel (separable phasor)",
            3: "rad_fused_kernel (single launch: pack + direct phasor + grid-wide ordered reduction)"}
 FLOPS_PER_EVAL = {1: {0: 43.25, 1: 43.25, 2: 47.6}, 2: {0: 20.19, 1: 20.19, 2: 26.63}, 3: {0: 43.25, 1: 43.25, 2: 47.6},
-                  "2c": {0: 19.06, 1: 19.06, 2: 24.38}}
+                  "2c": {0: 19.06, 1: 19.06, 2: 24.38}, "2w": {0: 19.31, 1: 19.31}}
 FP64_INSTR_PER_EVAL = {1: {0: 24.6, 1: 24.6, 2: 26.9}, 2: {0: 11.75, 1: 11.75, 2: 15.19}, 3: {0: 24.6, 1: 24.6, 2: 26.9},
-                       "2c": {0: 11.09, 1: 11.09, 2: 13.88}}
+                       "2c": {0: 11.09, 1: 11.09, 2: 13.88}, "2w": {0: 11.19, 1: 11.19}}
 
 
 def work_key(plan):
     """Key into the two tables above for the kernel of a plan's first part."""
-    return "2c" if plan["kernel"] == 2 and plan.get("cluster", 1) == 2 else plan["kernel"]
+    if plan["kernel"] == 2 and plan.get("cluster", 1) >= 2:
+        return "2c" if plan["cluster"] == 2 else "2w"
+    return plan["kernel"]
 FP64_SPEC_TFLOPS = 148 * 64 * 2 * 1.965e9 / 1e12      # 148 SM x 64 FMA lanes x 2 x 1.965 GHz
 MODELS = ["classical", "spin0", "spin1/2"]
 # dram__bytes_read.sum + dram__bytes_write.sum per main-kernel launch from the committed ncu --set full captures
@@ -359,8 +362,8 @@ class Bench:
             name = f"{KERNELS[2]} on {plan['interior_x']} x {plan['interior_y']} angles + {KERNELS[1]} on the rest"
         else:
             flops, instr, name = evals * FLOPS_PER_EVAL[wk][model], evals * FP64_INSTR_PER_EVAL[wk][model], KERNELS[k]
-        if wk == "2c":
-            name += ", cluster pairs sharing the T table"
+        if wk in ("2c", "2w"):
+            name += ", cluster pairs sharing the T table" if wk == "2c" else ", cluster pairs sharing the F table"
         achieved = flops / main_s
         key = f"{wl.name}|{k}"
         return {"bound": "alu", "kernel": name, "achieved": achieved / 1e12, "peak": self.peak / 1e12, "unit": "TFLOP/s",

@@ -292,7 +292,8 @@ int rad_plan_kernel(int32_t count, int64_t n_max, int32_t n_omega, int32_t n_thx
  * rest of the angle plane), plan[7] angle columns and plan[8] angle rows of the separable interior (0 if none),
  * plan[9] kernel launches of the whole call, plan[10] CTAs per thread-block cluster of the first part (2: the
  * separable kernel runs as cluster pairs on neighbouring angle tiles that share one phasor table through
- * distributed shared memory -- whenever the part has an even number of theta_y tiles; else 1).
+ * distributed shared memory -- whenever the part has an even number of theta_y tiles; 3: pairs on neighbouring
+ * omega tiles that share the integrand table, for an odd theta_y tile count with 4 accumulators per point; else 1).
  * plan: HOST array of at least 11 entries. */
 int rad_plan_describe(int32_t count, int64_t n_max, int32_t n_omega, int32_t n_thx, int32_t n_thy,
                       rad_model model, int32_t kernel, int32_t *plan);

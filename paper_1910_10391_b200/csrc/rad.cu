@@ -676,8 +676,11 @@ static cudaError_t launch_main(const MainParams &mp, dim3 grid, cudaStream_t st)
 
 template <int NC, int WY>
 static cudaError_t launch_sep(const MainParams &mp, dim3 grid, cudaStream_t st) {
-    if (mp.cl == 2) {         // cluster pairs along the y tiles (thread-block cluster of 2 CTAs on neighbouring SMs)
-        const cudaError_t a = ensure_smem(rad_sep_kernel<NC, WY, 2>, NC == 6 ? 7 : 6, SepShape<NC, WY>::SMEM);
+    if (mp.cl >= 2) {         // cluster pairs along the y (omega) tiles: thread-block clusters of 2 CTAs on neighbouring SMs
+        constexpr int CLW = NC == 4 ? 3 : 2;          // (pairs along omega exist for 4 accumulators per point only)
+        const bool along_w = mp.cl == 3 && NC == 4;
+        const cudaError_t a = along_w ? ensure_smem(rad_sep_kernel<NC, WY, CLW>, 8, SepShape<NC, WY>::SMEM)
+                                      : ensure_smem(rad_sep_kernel<NC, WY, 2>, NC == 6 ? 7 : 6, SepShape<NC, WY>::SMEM);
         if (a != cudaSuccess) return a;
         cudaLaunchConfig_t cfg = {};
         cfg.gridDim = grid; cfg.blockDim = dim3(SepRegs<NC>::THREADS); cfg.dynamicSmemBytes = SepShape<NC, WY>::SMEM;
@@ -687,7 +690,8 @@ static cudaError_t launch_sep(const MainParams &mp, dim3 grid, cudaStream_t st) 
         at[0].val.clusterDim.x = 2; at[0].val.clusterDim.y = 1; at[0].val.clusterDim.z = 1;
         cfg.attrs = at; cfg.numAttrs = 1;
         ++g_launches;
-        return cudaLaunchKernelEx(&cfg, rad_sep_kernel<NC, WY, 2>, mp);
+        return along_w ? cudaLaunchKernelEx(&cfg, rad_sep_kernel<NC, WY, CLW>, mp)
+                       : cudaLaunchKernelEx(&cfg, rad_sep_kernel<NC, WY, 2>, mp);
     }
     const cudaError_t a = ensure_smem(rad_sep_kernel<NC, WY, 1>, NC == 6 ? 3 : 2, SepShape<NC, WY>::SMEM);
     if (a != cudaSuccess) return a;

@@ -44,7 +44,9 @@ struct Part {
     Plan plan;
     size_t off_partial;
     int cl;                   // separable kernel: 2 = launched as cluster pairs of CTAs on neighbouring y tiles that
-                              // share the T table through distributed shared memory (needs an even y tile count)
+                              // share the T table through distributed shared memory (needs an even y tile count);
+                              // 3 = pairs on neighbouring omega tiles that share the F table (4 accumulators per
+                              // point, even omega tile count, cube output); 1 = single CTAs
 };
 
 struct CallPlan {
@@ -213,6 +215,7 @@ static inline CallPlan plan_call(int count, int64_t n_max, int n_omega, int n_th
         if (pt.kernel == K_SEP) {
             const int ty = nc == 6 ? 8 : 16;
             if (((pt.n_thy + ty - 1) / ty) % 2 == 0) pt.cl = 2;
+            else if (nc == 4 && !angular && ((n_omega + 15) / 16) % 2 == 0) pt.cl = 3;
         }
 #endif
     }

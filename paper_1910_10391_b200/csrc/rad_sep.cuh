@@ -119,7 +119,8 @@ struct SepCoord {
     int iw0, ix0, iy0;               // first omega / x / y index of this thread's points
     int lw, lx, ly, ww, wx;
     // cl = 2: the CTAs of a cluster pair (blocks 2k, 2k + 1) own neighbouring y tiles of one (omega, x) tile,
-    // so that they share the T table (rad_sep_kernel); the y tile count is even then.
+    // so that they share the T table (rad_sep_kernel); the y tile count is even then.  cl = 3: neighbouring omega
+    // tiles of one angle tile (shared F table); the omega tile count is even then.
     __device__ __forceinline__ SepCoord(int block, int tid, int n_thx, int n_thy, int cl) {
         const int ntx = (n_thx + 15) / 16, nty = (n_thy + 4 * WY - 1) / (4 * WY);
         if (cl == 2) {
@@ -127,6 +128,11 @@ struct SepCoord {
             bx = (rest % ntx) * 16;
             by = (((rest / ntx) % half) * 2 + (block & 1)) * 4 * WY;
             bw = (rest / (ntx * half)) * 16;
+        } else if (cl == 3) {                         // pairs on neighbouring OMEGA tiles of one angle tile (shared F table)
+            const int rest = block >> 1;
+            bx = (rest % ntx) * 16;
+            by = ((rest / ntx) % nty) * 4 * WY;
+            bw = ((rest / (ntx * nty)) * 2 + (block & 1)) * 16;
         } else {
             bx = (block % ntx) * 16;
             by = ((block / ntx) % nty) * 4 * WY;
@@ -277,12 +283,16 @@ struct SepCursor {
 // local half with an ordinary store, the peer's with st.async, whose bytes the peer's full[] barrier counts
 // (expect_tx posted with the arrival of the peer's first producer warp).  empty[] counts the consumer warps of both
 // CTAs, so a producer overwrites a buffer only when both CTAs have read it.  Y, F, H stay private.  Both CTAs step through the same (trajectory, chunk,
+// CL = 3 (4 accumulators per point only): the pair owns neighbouring OMEGA tiles of one angle tile instead -- for
+// grids with an odd number of y tiles, such as config 4's single 16 x 16 angle tile -- and what it shares is the
+// omega-independent integrand table F, by the same mechanism.
 // sub-block) sequence, so the protocol is symmetric; a cluster barrier at the start (barriers initialised before the
 // peer arrives on them) and at the end (no CTA leaves while the peer may still store into it) frames it.
 template <int NC, int WY, int CL>
 __global__ void __launch_bounds__(SepRegs<NC>::THREADS, 1)
 rad_sep_kernel(const MainParams P) {
-    static_assert(CL == 1 || CL == 2, "cluster pair or single CTA");
+    static_assert(CL == 1 || CL == 2 || (CL == 3 && NC == 4), "single CTA, pair sharing T, pair sharing F");
+    constexpr bool PAIR = CL >= 2;
     using SH = SepShape<NC, WY>;
     constexpr int YN = SH::YN, EV = SH::EV, S = SEP_S, NB = SEP_NB;
     extern __shared__ __align__(128) unsigned char smem_raw[];
@@ -298,12 +308,12 @@ rad_sep_kernel(const MainParams P) {
 
     if (tid == 0) {
         for (int s = 0; s < SEP_STAGES; ++s) mbar_init(&bars[s], 1);
-        for (int b = 0; b < NB; ++b) { mbar_init(&full[b], SepRegs<NC>::NPROD / 32); mbar_init(&empty[b], CL * SEP_CONS / 32); }
+        for (int b = 0; b < NB; ++b) { mbar_init(&full[b], SepRegs<NC>::NPROD / 32); mbar_init(&empty[b], (PAIR ? 2 : 1) * SEP_CONS / 32); }
         mbar_fence_init();
     }
     __syncthreads();
     uint32_t peer = 0, my_rank = 0;
-    if (CL == 2) {
+    if (PAIR) {
         cluster_sync_all();                           // the peer's barriers are initialised
         my_rank = cluster_ctarank();
         peer = my_rank ^ 1u;
@@ -322,16 +332,18 @@ rad_sep_kernel(const MainParams P) {
         const int pe = pt % NE, hs = pt / NE;            // entry slot, sample group
         constexpr bool SPLIT = YN < NE;
         static_assert(256 % NE == 0 && (SPLIT ? 2 * YN == NE : YN % NE == 0), "producer entry assignment");
-        static_assert((256 / NE) % CL == 0, "the T entries of a thread are dealt out to the CTAs of the pair");
-        constexpr int RT = 256 / NE / CL, RY = SPLIT ? 1 : YN / NE;         // CL = 2: entry slots r * CL + rank
+        constexpr int TS = CL == 2 ? 2 : 1, FS = CL == 3 ? 2 : 1;           // CTAs that share the T / the F entries
+        static_assert((256 / NE) % TS == 0 && (SPLIT ? FS == 1 : (YN / NE) % FS == 0),
+                      "the shared entries of a thread are dealt out to the CTAs of the pair");
+        constexpr int RT = 256 / NE / TS, RY = SPLIT ? 1 : YN / NE, RF = RY / FS;   // shared: entry slots r * 2 + rank
         const bool doY = !SPLIT || pe < YN, doF = !SPLIT || pe >= YN;
         const int ptF = SPLIT ? (pe >= YN ? pe - YN : 0) : pe, ptY = SPLIT ? (pe < YN ? pe : 0) : pe;
-        double omT[RT], nxT[RT], omY[RY], nyY[RY], nxF[RY], nyF[RY], hF[RY];
-        uint32_t peer_T = 0, peer_full = 0;           // the peer's T ring and full[] barriers (shared::cluster addresses)
-        if (CL == 2) { peer_T = map_to_cta(smem_u32(Tt), peer); peer_full = map_to_cta(smem_u32(full), peer); }
+        double omT[RT], nxT[RT], omY[RY], nyY[RY], nxF[RF], nyF[RF], hF[RF];
+        uint32_t peer_T = 0, peer_full = 0;           // the peer's T (F) ring and full[] barriers (shared::cluster addresses)
+        if (PAIR) { peer_T = map_to_cta(smem_u32(CL == 2 ? Tt : Ft), peer); peer_full = map_to_cta(smem_u32(full), peer); }
 #pragma unroll
         for (int r = 0; r < RT; ++r) {
-            const int b = pe + (r * CL + (int)my_rank) * NE;
+            const int b = pe + (r * TS + (CL == 2 ? (int)my_rank : 0)) * NE;
             const int iw = co.bw + 4 * (b >> 6) + 2 * (b & 1) + ((b >> 4) & 1);
             const int ix = co.bx + 8 * ((b >> 5) & 1) + 2 * ((b >> 1) & 3) + ((b >> 3) & 1);
             omT[r] = P.omega[min(iw, P.n_omega - 1)];
@@ -347,8 +359,11 @@ rad_sep_kernel(const MainParams P) {
                 omY[r] = P.omega[min(iw, P.n_omega - 1)];
                 nyY[r] = P.thy[min(iy, P.n_thy - 1)];
             }
+        }
+#pragma unroll
+        for (int r = 0; r < RF; ++r) {
             {
-                const int b = ptF + r * NE;
+                const int b = ptF + (r * FS + (CL == 3 ? (int)my_rank : 0)) * NE;
                 const int q = b >> 4, m = q % WY, j = (q / WY) & 1, wx = (q / WY) >> 1;
                 const int ix = co.bx + 8 * wx + 2 * ((b >> 2) & 3) + j;
                 const int iy = co.by + WY * (b & 3) + m;
@@ -422,7 +437,7 @@ rad_sep_kernel(const MainParams P) {
                     for (int r = 0; r < RT; ++r) {
                         const double dT = fma(-nxT[r], r89.x, fma(hxT[r], r67.y, r67.x));
                         const double2 ph = phasor_full(fma(whT[r], dT, p0T[r]));
-                        const int e = row * 256 + pe + (r * CL + (int)my_rank) * NE;
+                        const int e = row * 256 + pe + (r * TS + (CL == 2 ? (int)my_rank : 0)) * NE;
                         Tt[e] = ph;
                         if (CL == 2) st_async_v2(peer_T + (uint32_t)e * 16u, ph, peer_full + (uint32_t)buf * 8u);
                     }
@@ -438,7 +453,7 @@ rad_sep_kernel(const MainParams P) {
                     const double2 r23 = *reinterpret_cast<const double2 *>(rec + 2);   // vy, w ax
                     const double2 r45 = *reinterpret_cast<const double2 *>(rec + 4);   // w ay, w az
 #pragma unroll
-                    for (int r = 0; r < RY; ++r) {       // a2: eqs. (3), (4), (6), (12), times the weight
+                    for (int r = 0; r < RF; ++r) {       // a2: eqs. (3), (4), (6), (12), times the weight
                         const double D = r01.x - hF[r];
                         const double ux = nxF[r] - r01.y, uy = nyF[r] - r23.x;
                         const double bx = fma(nyF[r], uy, D);
@@ -447,15 +462,17 @@ rad_sep_kernel(const MainParams P) {
                         const double gq = inv_square(q);
                         const double s1 = fma(nyF[r], r45.x, r45.y);
                         const double s2 = fma(nxF[r], r23.y, r45.y);
-                        Ft[row * YN + ptF + r * NE] = make_double2(fma(s1, ux, -(bx * r23.y)) * gq,
-                                                                      fma(s2, uy, -(by * r45.x)) * gq);
-                        if (NC == 6) Hh[row * YN + ptF + r * NE] = fma(nxF[r], r23.y, s1) * gq;
+                        const int e = row * YN + ptF + (r * FS + (CL == 3 ? (int)my_rank : 0)) * NE;
+                        const double2 fv = make_double2(fma(s1, ux, -(bx * r23.y)) * gq, fma(s2, uy, -(by * r45.x)) * gq);
+                        Ft[e] = fv;
+                        if (CL == 3) st_async_v2(peer_T + (uint32_t)e * 16u, fv, peer_full + (uint32_t)buf * 8u);
+                        if (NC == 6) Hh[e] = fma(nxF[r], r23.y, s1) * gq;
                     }
                 }
                 __syncwarp();
                 if ((pt & 31) == 0) {
-                    // the peer's half of the T table arrives asynchronously: S samples x 256 / CL entries x 16 bytes
-                    if (CL == 2 && pt == 0) mbar_expect_tx(&full[buf], S * (256 / CL) * 16);
+                    // the peer's half of the shared table arrives asynchronously: S samples x 128 entries x 16 bytes
+                    if (PAIR && pt == 0) mbar_expect_tx(&full[buf], S * ((CL == 2 ? 256 : YN) / 2) * 16);
                     else mbar_arrive(&full[buf]);
                 }
                 ++g;
@@ -466,7 +483,7 @@ rad_sep_kernel(const MainParams P) {
             producer_bar_sync<NPROD>();
             if (pt == 0) produce();
         }
-        if (CL == 2) cluster_sync_all();              // (matches the consumers' barrier at the end of the kernel)
+        if (PAIR) cluster_sync_all();                 // (matches the consumers' barrier at the end of the kernel)
         return;
     }
 
@@ -474,7 +491,7 @@ rad_sep_kernel(const MainParams P) {
     reg_alloc<SepRegs<NC>::CONS>();
     const SepCoord<WY> co(blockIdx.x, tid, P.n_thx, P.n_thy, CL);
     uint32_t peer_empty = 0;
-    if (CL == 2) peer_empty = map_to_cta(smem_u32(empty), peer);
+    if (PAIR) peer_empty = map_to_cta(smem_u32(empty), peer);
     const int64_t gid = (int64_t)blockIdx.x * SEP_CONS + tid;
     // read offsets (entries) of this thread inside one sample's tables
     const int rT = (co.ww * 2 + co.wx) * 32 + co.lx * 2 + co.lw;          // + (i*2 + j) * 8
@@ -557,7 +574,10 @@ rad_sep_kernel(const MainParams P) {
             // (The 64 accumulators of the 4-per-point variant leave ptxas so few registers that it renames
             // accumulators and moves them back: 106-194 IMAD.MOV per 1007 FP64 instructions of the loop, depending on
             // unrelated code around it; staged or not changes the throughput by +-1 %.)
-            constexpr bool STAGED = true;
+#ifndef RAD_SEP_STAGED4
+#define RAD_SEP_STAGED4 true
+#endif
+            constexpr bool STAGED = NC == 6 || RAD_SEP_STAGED4;
             if (STAGED) products(0, qr, qi);
 #pragma unroll
             for (int g = 0; g < G; ++g) {
@@ -591,7 +611,7 @@ rad_sep_kernel(const MainParams P) {
         __syncwarp();
         if ((tid & 31) == 0) {
             mbar_arrive(&empty[buf]);
-            if (CL == 2) mbar_arrive_remote(peer_empty + (uint32_t)buf * 8u);
+            if (PAIR) mbar_arrive_remote(peer_empty + (uint32_t)buf * 8u);
         }
         ++g;
         if (--todo == 0) {
@@ -648,7 +668,7 @@ rad_sep_kernel(const MainParams P) {
             P.ang_partial[(int64_t)blockIdx.x * 16 + tid] = sum;
         }
     }
-    if (CL == 2) cluster_sync_all();                  // the peer may still store T entries / arrive here until it is done
+    if (PAIR) cluster_sync_all();                     // the peer may still store table entries / arrive here until it is done
 }
 
 // angular spectrum, second pass for the separable kernel: spec[i_w] (+)= d_solid * sum over the angle tiles of

@@ -453,7 +453,21 @@ def test_sep_cluster_pairs_time_and_trajectory_split(sep_kernel, oracle_mod):
     assert torch.equal(cube, again)
     w, nx, ny = oracle_mod.grid_points(wl.omega, thx, wl.thy)
     assert_parity(cube.cpu().numpy(), oracle_mod.points(wl.traj, w, nx, ny, CL, 0.0), label="cluster time split")
-    assert rad.rad_plan_describe(1, 1500, 20, 5, 40, CL, 2)["cluster"] == 1        # 3 y tiles: single CTAs
+    # 3 y tiles: no y neighbour for every tile.  Classical / spin-0 grids with an even number of omega tiles then pair
+    # along omega and share the F table (cluster code 3); spin-1/2 and odd omega tile counts run as single CTAs.
+    assert rad.rad_plan_describe(1, 1500, 20, 5, 40, CL, 2)["cluster"] == 3
+    assert rad.rad_plan_describe(1, 1500, 20, 5, 40, SH, 2)["cluster"] == 1
+    assert rad.rad_plan_describe(1, 1500, 40, 5, 40, CL, 2)["cluster"] == 1
+    thy3 = np.linspace(wl.thy[0], wl.thy[-1], 40)
+    g3 = [torch.from_numpy(np.ascontiguousarray(a)).cuda() for a in (wl.omega, thx, thy3)]
+    for spin in (None, 0):                             # time split through the omega pairs, classical and spin-0
+        lam3 = 0.4 / wl.omega.max()
+        cube = rad.rad_classical(tr, *g3) if spin is None else rad.rad_semiclassical(tr, *g3, 0, lam3)
+        again = rad.rad_classical(tr, *g3) if spin is None else rad.rad_semiclassical(tr, *g3, 0, lam3)
+        assert torch.equal(cube, again)
+        w, nx, ny = oracle_mod.grid_points(wl.omega, thx, thy3)
+        assert_parity(cube.cpu().numpy(), oracle_mod.points(wl.traj, w, nx, ny, CL if spin is None else S0,
+                                                            0.0 if spin is None else lam3), label="omega pairs time split")
 
     we = workloads.make("cfg4", count=40, n=260, n_omega=9, n_th=11, seed0=1234)
     thx = we.thx[:6].copy()
@@ -470,6 +484,14 @@ def test_sep_cluster_pairs_time_and_trajectory_split(sep_kernel, oracle_mod):
     w, nx, ny = oracle_mod.grid_points(we.omega, thx, we.thy)
     assert_parity(cube.cpu().numpy(), oracle_mod.ensemble_points(we.batch, nvec, w, nx, ny, SH, lam),
                   label="cluster trajectory split")
+    # the same ragged ensemble, classical, on 20 omegas x one angle tile: omega pairs in the trajectory split
+    we2 = workloads.make("cfg4", count=40, n=260, n_omega=20, n_th=7, seed0=1234)
+    plan = rad.rad_plan_describe(40, 260, 20, 7, 7, CL, 2)
+    assert plan["cluster"] == 3 and plan["mode"] == 1
+    cube = rad.rad_ensemble_sum(dev_dict(we2.batch), nvec, *dev_grid(we2))
+    w, nx, ny = oracle_mod.grid_points(we2.omega, we2.thx, we2.thy)
+    assert_parity(cube.cpu().numpy(), oracle_mod.ensemble_points(we2.batch, nvec, w, nx, ny),
+                  label="omega pairs trajectory split")
 
 
 # ------------------------------------------------------------------ edge cases through the separable kernel too
