@@ -1073,14 +1073,24 @@ int rad_ensemble_sum_host(const rad_traj_batch *b, const rad_grid *g, rad_model 
     PoolScratch pool;
     pool.p = dev; pool.st = st;
     const double *d[11];
-    for (int i = 0; i < 11; ++i) {
-        d[i] = dev + i * tot;
-        CK(cudaMemcpyAsync(dev + i * tot, src[i], tot * sizeof(double), cudaMemcpyHostToDevice, st));
+    // Arrays that follow one another in host memory (a caller that keeps its SoA block in one allocation) go over in
+    // ONE copy: for a small problem the eleven + three separate copies cost more than the kernel (config 1: 14 copies
+    // ~ 85 us against a 47 us kernel).
+    for (int i = 0; i < 11;) {
+        int j = i;
+        while (j + 1 < 11 && src[j + 1] == src[j] + tot) ++j;
+        CK(cudaMemcpyAsync(dev + i * tot, src[i], (size_t)(j - i + 1) * tot * sizeof(double), cudaMemcpyHostToDevice, st));
+        for (int k = i; k <= j; ++k) d[k] = dev + k * tot;
+        i = j + 1;
     }
     double *gw = dev + 11 * tot, *gx = gw + g->n_omega, *gy = gx + g->n_thx, *dout = gy + g->n_thy;
-    CK(cudaMemcpyAsync(gw, g->omega, g->n_omega * sizeof(double), cudaMemcpyHostToDevice, st));
-    CK(cudaMemcpyAsync(gx, g->thx, g->n_thx * sizeof(double), cudaMemcpyHostToDevice, st));
-    CK(cudaMemcpyAsync(gy, g->thy, g->n_thy * sizeof(double), cudaMemcpyHostToDevice, st));
+    if (g->thx == g->omega + g->n_omega && g->thy == g->thx + g->n_thx) {
+        CK(cudaMemcpyAsync(gw, g->omega, ng * sizeof(double), cudaMemcpyHostToDevice, st));
+    } else {
+        CK(cudaMemcpyAsync(gw, g->omega, g->n_omega * sizeof(double), cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(gx, g->thx, g->n_thx * sizeof(double), cudaMemcpyHostToDevice, st));
+        CK(cudaMemcpyAsync(gy, g->thy, g->n_thy * sizeof(double), cudaMemcpyHostToDevice, st));
+    }
     if (accumulate) CK(cudaMemcpyAsync(dout, out, M * sizeof(double), cudaMemcpyHostToDevice, st));
     rad_traj_batch db{b->count, b->stride, b->n, d[0], d[1], d[2], d[3], d[4], d[5], d[6], d[7], d[8], d[9], d[10]};
     rad_grid dg{g->n_omega, g->n_thx, g->n_thy, gw, gx, gy};

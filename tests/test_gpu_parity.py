@@ -240,6 +240,20 @@ def test_host_entry_points(rad, oracle_mod):
     both = rad.rad_ensemble_sum_host({k: np.ascontiguousarray(v[2:]) for k, v in we.batch.items()}, we.n[2:],
                                      we.omega, we.thx, we.thy, accumulate=True, out=part)
     assert_parity(both, ref, label="host ensemble accumulate")
+    # SoA arrays that follow one another in one host allocation go over in one transfer (partly adjacent: the first
+    # seven fields in one block, the rest separate; grid arrays in one block): bit-identical results
+    block = np.empty((7,) + we.batch["t"].shape)
+    mixed = {}
+    for i, k in enumerate(rad.FIELDS):
+        if i < 7:
+            block[i] = we.batch[k]
+            mixed[k] = block[i]
+        else:
+            mixed[k] = we.batch[k].copy()
+    gb = np.concatenate([we.omega, we.thx, we.thy])
+    nw, nx_ = len(we.omega), len(we.thx)
+    again = rad.rad_ensemble_sum_host(mixed, we.n, gb[:nw], gb[nw:nw + nx_], gb[nw + nx_:])
+    assert np.array_equal(again, cube)
 
 
 # ------------------------------------------------------------------ angular sum (NEXT-1)
