@@ -12,8 +12,12 @@
 //   rad_finalize_kernel  a6/a7  ordered reduction of time-split amplitudes / trajectory-split
 //                               spectra
 //   rad_angular_sum_kernel      sum of the cube over angles
-//   rad_sep_kernel (rad_sep.cuh) a0-a7 again for tensor grids that fill its tiles: the phasor of eq. (7)
-//                               factorised into T(omega, n_x) Y(omega, n_y), warp-specialised CTA
+//   rad_sep_kernel (rad_sep.cuh) a0-a7 again for tensor grids that fill its tiles (the default path): the phasor of
+//                               eq. (7) factorised into T(omega, n_x) Y(omega, n_y), warp-specialised CTAs in
+//                               thread-block cluster pairs that share a table through distributed shared memory
+//   rad_fused_kernel (rad_fused.cuh) a0-a6 in ONE cooperative launch for one short trajectory on a small grid
+//   rad_ang_final_*_kernel      second pass of the angular spectrum formed in the main kernels' epilogue (no cube)
+//   (launch planning: rad_plan.h)
 //   rad_sum_cubes_kernel        ordered sum of partial cubes (ensemble shards)
 //   rad_traj_kernel (rad_traj.cuh)  synthetic-well trajectories on the device
 #include <atomic>

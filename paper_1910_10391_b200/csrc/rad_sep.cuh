@@ -9,8 +9,11 @@
 // Per eval what remains is one complex multiply and the complex accumulation (8 or 10 FP64
 // instructions instead of 24 or 26).
 //
-// CTA = 384 threads, warp-specialised (one CTA per SM):
-//   warps 8-11  PRODUCERS (phase A): wait for trajectory chunks (TMA ring), build the T, Y, F (H)
+// CTA = 256 consumer + 128 (4 accumulators per point) or 256 (6) producer threads, warp-specialised, one CTA per SM,
+// launched as thread-block CLUSTER PAIRS wherever the tile counts allow: the two CTAs of a pair own neighbouring
+// theta_y tiles (same T table) or neighbouring omega tiles (same F table), compute half of the shared table each and
+// store the peer's copy through distributed shared memory (st.async, counted on the peer's mbarrier); see the kernel.
+//   warps 8-..  PRODUCERS (phase A): wait for trajectory chunks (TMA ring), build the T, Y, F (H)
 //               tables of SEP_S samples per sub-block into a ring of SEP_NB table buffers in
 //               shared memory (16-byte entries: (re, im) of T and Y, (w f_x, w f_y) of F).
 //   warps 0-7   CONSUMERS (phase B): thread tile 2 omega x 2 n_x x WY n_y (WY = 4 with 4
