@@ -64,7 +64,10 @@ rad_fused_kernel(const FusedParams P) {
     const int wg_lo = (int)(min((int64_t)blockIdx.x * FUSED_TPB, T - 1) / A);
     const int wg_hi = (int)(min((int64_t)blockIdx.x * FUSED_TPB + FUSED_TPB - 1, T - 1) / A);
     for (int i = tid; i < (wg_hi - wg_lo + 1) * W; i += FUSED_TPB) {
-        const dd wt = omega_star_turns(P.omega[min(wg_lo * W + i, P.n_omega - 1)], P.lam);
+        // (classical: omega* = omega, no divisions -- half a microsecond of a 47 us kernel.  Only here: the same
+        // branch inside omega_star_turns costs the separable kernel's producers 2-14 %)
+        const double om = P.omega[min(wg_lo * W + i, P.n_omega - 1)];
+        const dd wt = P.lam == 0.0 ? dd_mul_d(dd{INV_2PI_HI, INV_2PI_LO}, om) : omega_star_turns(om, P.lam);
         wt_sm[i] = make_double2(wt.hi, wt.lo);
     }
     __syncthreads();
