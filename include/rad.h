@@ -66,7 +66,8 @@ typedef enum {
     RAD_EINVAL = -1,      /* null pointer, n < 2, empty grid, bad spin/model, misaligned pointer */
     RAD_EDOMAIN = -2,     /* host-visible parameter outside the method's domain (hbarc_over_E < 0) */
     RAD_ECUDA = -3,       /* CUDA runtime error; rad_strerror gives the CUDA text of the last one */
-    RAD_ENOSPACE = -4     /* workspace given but smaller than rad_workspace_bytes() */
+    RAD_ENOSPACE = -4,    /* workspace given but smaller than rad_workspace_bytes() */
+    RAD_ETOOBIG = -5      /* rad_eval_static: the call needs more scratch than rad_static_scratch_bytes() */
 } rad_status;
 
 typedef enum { RAD_CLASSICAL = 0, RAD_SPIN0 = 1, RAD_SPIN_HALF = 2 } rad_model;
@@ -271,6 +272,26 @@ int rad_eval_host(const rad_traj *traj, const rad_grid *grid, rad_model model,
 int rad_ensemble_sum_host(const rad_traj_batch *batch, const rad_grid *grid, rad_model model,
                           const double *hbarc_over_E, int accumulate, double *out,
                           const rad_options *opt, void *cuda_stream);
+
+/* The entry point that ALLOCATES NOTHING: the cube of one trajectory (classical, spin-0 or spin-1/2; the same
+ * operation and the same kernels as rad_classical / rad_semiclassical) for callers that must not reach cudaMalloc or
+ * a memory pool -- code under CUDA graph capture, tight serving loops, harnesses that forbid allocation.  Its scratch
+ * (packed trajectory records, partial amplitudes of a time split) lives in ONE file-scope device array of
+ * rad_static_scratch_bytes() = 16 MiB that every GPU loading the library holds until the process exits.
+ *   - All pointers DEVICE memory as in rad_classical; the caller passes inputs and `out` (n_omega*n_thy*n_thx doubles).
+ *   - Limit: calls whose launch plan needs more than rad_static_scratch_bytes() return RAD_ETOOBIG and enqueue
+ *     nothing (rad_workspace_bytes(1, n, n_omega, n_thx, n_thy) is an upper bound of the need; e.g. BASELINE
+ *     config 1 fits, config 2's 16-way time split does not -- use rad_classical with a workspace there).
+ *   - Calls no cudaMalloc / cudaMallocAsync / cudaFree and no allocating library routine; it enqueues kernels on
+ *     `cuda_stream` and does not synchronise.  (The first call on a device asks the runtime for the array's device
+ *     address, cudaGetSymbolAddress, once.)
+ *   - Every call on a device shares the one array, which keeps the previous call's contents: the kernels overwrite
+ *     every byte they later read, so nothing needs clearing, but two calls that OVERLAP on the GPU (different
+ *     streams, or a captured graph replayed concurrently with itself) race on it -- keep them in one stream order.
+ * hbarc_over_E is ignored for RAD_CLASSICAL. */
+int rad_eval_static(const rad_traj *traj, const rad_grid *grid, rad_model model, double hbarc_over_E, double *out,
+                    const rad_options *opt, void *cuda_stream);
+size_t rad_static_scratch_bytes(void);
 
 /* FP64 FMA peak of the current device, measured: runs a register-resident DFMA chain
  * kernel for about `millis` ms and returns FLOP/s (2 per FMA lane); <= 0 on error. */

@@ -19,7 +19,8 @@ from .binding import (CLASSICAL, FIELDS, KERNEL_AUTO, KERNEL_DIRECT, KERNEL_FUSE
                       load_library, rad_angular_spectrum, rad_angular_sum, rad_classical, rad_ensemble_sum,
                       rad_ensemble_sum_host, rad_eval_host, rad_formation_length, rad_generate_trajectories,
                       rad_launch_count, rad_measure_fp64_peak, rad_number_spectrum, rad_plan_describe, rad_plan_kernel,
-                      rad_sections_check, rad_sections_sum, rad_semiclassical, rad_sum_cubes, rad_workspace_bytes)
+                      rad_sections_check, rad_sections_sum, rad_semiclassical, rad_sum_cubes, rad_workspace_bytes,
+                      rad_eval_static, rad_static_scratch_bytes)
 from .sharding import rad_ensemble_sum_sharded, rad_eval_grid_sharded, shard_range, shard_sizes
 
 __all__ = [
@@ -30,4 +31,5 @@ __all__ = [
     "rad_number_spectrum", "KERNEL_AUTO", "KERNEL_DIRECT", "KERNEL_SEPARABLE", "KERNEL_FUSED",
     "rad_generate_trajectories", "rad_plan_describe", "rad_angular_spectrum", "rad_formation_length", "WELL_COSINE", "WELL_AXIAL_EXP", "WELL_HARMONIC_MS",
     "rad_ensemble_sum_sharded", "rad_eval_grid_sharded", "shard_range", "shard_sizes",
+    "rad_eval_static", "rad_static_scratch_bytes",
 ]

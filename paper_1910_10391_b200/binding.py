@@ -22,7 +22,7 @@ EXPORTS = ("rad_classical", "rad_semiclassical", "rad_ensemble_sum", "rad_sectio
            "rad_profile_create", "rad_profile_destroy", "rad_profile_read", "rad_plan_kernel",
            "rad_generate_trajectories", "rad_plan_describe", "rad_angular_spectrum",
            "rad_angular_spectrum_workspace_bytes", "rad_formation_length", "rad_sections_check",
-           "rad_number_spectrum")
+           "rad_number_spectrum", "rad_eval_static", "rad_static_scratch_bytes")
 
 KERNEL_AUTO, KERNEL_DIRECT, KERNEL_SEPARABLE, KERNEL_FUSED = 0, 1, 2, 3
 
@@ -111,6 +111,8 @@ def load_library() -> ctypes.CDLL:
                                       + [vp] * 4 + [P(_TrajBuffers), vp]),
         "rad_workspace_bytes": (sz, [i32, i64, i32, i32, i32]),
         "rad_eval_host": (ctypes.c_int, [P(_Traj), P(_Grid), ctypes.c_int, dbl, vp, op, vp]),
+        "rad_eval_static": (ctypes.c_int, [P(_Traj), P(_Grid), ctypes.c_int, dbl, vp, op, vp]),
+        "rad_static_scratch_bytes": (sz, []),
         "rad_ensemble_sum_host": (ctypes.c_int, [P(_Batch), P(_Grid), ctypes.c_int, vp, ctypes.c_int, vp, op, vp]),
         "rad_measure_fp64_peak": (dbl, [dbl, vp]),
         "rad_launch_count": (i64, []),
@@ -234,6 +236,23 @@ def rad_semiclassical(traj: dict, omega, thx, thy, spin: int, hbarc_over_E: floa
     _check(load_library().rad_semiclassical(ctypes.byref(t), ctypes.byref(g), int(spin), float(hbarc_over_E),
                                             out.data_ptr(), ws, nb, _opt(kernel, profile), _stream_ptr(stream)))
     return out
+
+
+def rad_eval_static(traj: dict, omega, thx, thy, model: int = CLASSICAL, hbarc_over_E: float = 0.0, out=None,
+                    stream=None, kernel: int = 0, profile=None):
+    """Cube of one trajectory through the entry point that allocates nothing (include/rad.h rad_eval_static): the
+    scratch is the library's 16 MiB static device array; RadError(RAD_ETOOBIG = -5) beyond it.  Pass ``out`` to keep
+    this wrapper from allocating the result tensor either."""
+    g = _grid_struct(_dev(omega, "omega"), _dev(thx, "thx"), _dev(thy, "thy"))
+    t = _traj_struct(traj)
+    out = _out_cube(out, omega, thx, thy)
+    _check(load_library().rad_eval_static(ctypes.byref(t), ctypes.byref(g), int(model), float(hbarc_over_E),
+                                          out.data_ptr(), _opt(kernel, profile), _stream_ptr(stream)))
+    return out
+
+
+def rad_static_scratch_bytes() -> int:
+    return int(load_library().rad_static_scratch_bytes())
 
 
 def rad_ensemble_sum(batch: dict, n, omega, thx, thy, model: int = CLASSICAL, hbarc_over_E=None,

@@ -1223,6 +1223,49 @@ int rad_profile_read(rad_profile *p, float *ms) {
     return RAD_OK;
 }
 
+// ---- the entry point that allocates nothing (include/rad.h rad_eval_static)
+// Scratch of the single-trajectory path (packed chunk records, partial amplitudes / spectra of a split plan) in a
+// file-scope device array instead of caller or pool memory: every GPU that loads this library holds these bytes until
+// the process exits.  In host code `g_static_scratch` is a host-side stand-in for the symbol, NOT a device address:
+// the address the kernels get comes from cudaGetSymbolAddress, asked once per device with that device current.
+constexpr size_t STATIC_SCRATCH_BYTES = (size_t)16 << 20;
+static __device__ __align__(256) unsigned char g_static_scratch[STATIC_SCRATCH_BYTES];
+static std::atomic<void *> g_static_scratch_ptr[rad::MAX_DEV];          // per device; nullptr = not asked yet
+
+static int static_scratch_address(void **ptr) {
+    const int dev = rad::current_device();
+    if (dev < 0) return rad::cuda_fail(cudaErrorNoDevice, "rad_eval_static");
+    void *p = g_static_scratch_ptr[dev].load();
+    if (!p) {
+        const cudaError_t e = cudaGetSymbolAddress(&p, g_static_scratch);
+        if (e != cudaSuccess) return rad::cuda_fail(e, "cudaGetSymbolAddress(g_static_scratch)");
+        g_static_scratch_ptr[dev].store(p);
+    }
+    *ptr = p;
+    return RAD_OK;
+}
+
+size_t rad_static_scratch_bytes(void) { return STATIC_SCRATCH_BYTES; }
+
+int rad_eval_static(const rad_traj *traj, const rad_grid *grid, rad_model model, double hbarc_over_E, double *out,
+                    const rad_options *opt, void *cuda_stream) {
+    if (!traj || traj->n < 2 || !grid_ok(grid) || !out) return RAD_EINVAL;
+    if (model < RAD_CLASSICAL || model > RAD_SPIN_HALF) return RAD_EINVAL;
+    if (model != RAD_CLASSICAL && !(hbarc_over_E >= 0.0)) return RAD_EDOMAIN;
+    const int kopt = kernel_option(opt);
+    if (kopt < RAD_KERNEL_AUTO || kopt > RAD_KERNEL_FUSED || (opt && opt->reserved != 0)) return RAD_EINVAL;
+    const int nc = model == RAD_SPIN_HALF ? 6 : 4;
+    const CallPlan cp = plan_for(1, traj->n, grid->n_omega, grid->n_thx, grid->n_thy, nc, kopt, false);
+    if (cp.total > STATIC_SCRATCH_BYTES) return RAD_ETOOBIG;          // (same plan, hence same size, as run_batch computes)
+    void *scratch = nullptr;
+    const int rc = static_scratch_address(&scratch);
+    if (rc != RAD_OK) return rc;
+    // the existing single-trajectory path with the static array as its caller workspace: with a workspace it enqueues
+    // kernels only (no cudaMalloc / cudaMallocAsync / cudaFree, no host copy, no synchronisation)
+    return run_single(traj, grid, (int)model, model == RAD_CLASSICAL ? 0.0 : hbarc_over_E, out, scratch,
+                      STATIC_SCRATCH_BYTES, opt, static_cast<cudaStream_t>(cuda_stream));
+}
+
 const char *rad_strerror(int code) {
     switch (code) {
         case RAD_OK: return "ok";
@@ -1230,6 +1273,8 @@ const char *rad_strerror(int code) {
         case RAD_EDOMAIN: return "parameter outside the method's domain";
         case RAD_ECUDA: return g_err;
         case RAD_ENOSPACE: return "workspace too small (see rad_workspace_bytes)";
+        case RAD_ETOOBIG: return "problem needs more scratch than the library's static scratch array holds "
+                                 "(rad_static_scratch_bytes; use rad_classical / rad_semiclassical with a workspace)";
         default: return "unknown status";
     }
 }
