@@ -605,8 +605,12 @@ static int fused_resident() {
     int v = slot.load();
     if (v == 0) {
         int per_sm = 0;
-        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rad_fused_kernel<NC, RAD_DEG>, FUSED_TPB, FUSED_SMEM)
-            != cudaSuccess) { cudaGetLastError(); per_sm = 0; }
+        int per_sm_gen = 0;                          // (the smaller of the two instantiations: one number plans both)
+        if (cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, rad_fused_kernel<NC, RAD_DEG, false>, FUSED_TPB, FUSED_SMEM)
+                != cudaSuccess
+            || cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm_gen, rad_fused_kernel<NC, RAD_DEG, true>, FUSED_TPB,
+                                                             FUSED_SMEM) != cudaSuccess) { cudaGetLastError(); per_sm = 0; }
+        per_sm = std::min(per_sm, per_sm_gen);
         v = per_sm * sm_count();
         slot.store(v > 0 ? v : -1);
     }
@@ -707,8 +711,9 @@ static cudaError_t launch_sep(const MainParams &mp, dim3 grid, cudaStream_t st) 
 template <int NC>
 static cudaError_t launch_fused(FusedParams &fp, cudaStream_t st) {
     void *args[] = {&fp};
-    const cudaError_t e = cudaLaunchCooperativeKernel(reinterpret_cast<const void *>(rad_fused_kernel<NC, RAD_DEG>),
-                                                      dim3(fp.tiles, fp.slices), dim3(FUSED_TPB), args, FUSED_SMEM, st);
+    const void *fn = fp.l_x0 >= 0 ? reinterpret_cast<const void *>(rad_fused_kernel<NC, RAD_DEG, true>)
+                                  : reinterpret_cast<const void *>(rad_fused_kernel<NC, RAD_DEG, false>);
+    const cudaError_t e = cudaLaunchCooperativeKernel(fn, dim3(fp.tiles, fp.slices), dim3(FUSED_TPB), args, FUSED_SMEM, st);
     ++g_launches;
     return e;
 }
@@ -764,7 +769,7 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const int64
         fp.model = model; fp.accumulate = accumulate ? 1 : 0;
         fp.tiles = cp.fused_tiles; fp.slices = cp.fused_slices;
         fp.partial = reinterpret_cast<double *>(ws + cp.part[0].off_partial);
-        fp.out = out;
+        fp.out = out; fp.l_x0 = -1; fp.l_y0 = -1;
         prof_mark(prof, 0, st);
         prof_mark(prof, 1, st);
         const cudaError_t e = nc == 6 ? launch_fused<6>(fp, st) : launch_fused<4>(fp, st);
@@ -821,6 +826,23 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const int64
             mp.ang_groups = std::min((g->n_omega + W - 1) / W, (TPB + pt.angles - 1) / pt.angles + 1);
             mp.ang_partial = reinterpret_cast<double *>(ws + cp.off_ang);
         }
+        if (pt.f_tiles > 0) {                         // the rest of a two-part plan through the fused single-launch kernel
+            const int64_t o = off_host ? off_host[0] : 0;
+            FusedParams fp{};
+            fp.tr = rad_traj{n_host[0], b->t + o, b->dz + o, b->x + o, b->y + o, b->vx + o, b->vy + o, b->dvz + o,
+                             b->ax + o, b->ay + o, b->az + o, b->gamma + o};
+            fp.lam = mp.lam_single;
+            fp.omega = g->omega; fp.thx = g->thx; fp.thy = g->thy;
+            fp.n_omega = g->n_omega; fp.n_thx = pt.n_thx; fp.n_thy = pt.n_thy;
+            fp.model = model; fp.accumulate = accumulate ? 1 : 0;
+            fp.tiles = pt.f_tiles; fp.slices = pt.f_slices;
+            fp.partial = mp.partial;
+            fp.out = out; fp.l_x0 = pt.l_x0; fp.l_y0 = pt.l_y0; fp.out_nx = g->n_thx;
+            fp.out_plane = (int64_t)g->n_thx * g->n_thy;
+            const cudaError_t ef = nc == 6 ? launch_fused<6>(fp, st) : launch_fused<4>(fp, st);
+            if (ef != cudaSuccess) return cuda_fail(ef, "rad_fused_kernel");
+            continue;
+        }
         dim3 grid((unsigned)pl.tiles, (unsigned)pl.slices());
         cudaError_t e;
         if (pt.kernel == K_SEP) e = nc == 6 ? launch_sep<6, 2>(mp, grid, st) : launch_sep<4, 4>(mp, grid, st);
@@ -846,7 +868,7 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const int64
             ++g_launches;
             CK(cudaGetLastError());
             reduced = true;
-        } else if (pl.mode != MODE_DIRECT) {
+        } else if (pl.mode != MODE_DIRECT && pt.f_tiles == 0) {
             if (pt.kernel == K_SEP) {
                 if (nc == 6) rad_sep_finalize_kernel<6, 2><<<dim3(pl.tiles, 8), SEP_CONS, 0, st>>>(mp);
                 else rad_sep_finalize_kernel<4, 4><<<dim3(pl.tiles, 16), SEP_CONS, 0, st>>>(mp);

@@ -33,12 +33,25 @@ struct FusedParams {
     int tiles, slices;        // gridDim.x, gridDim.y
     double *partial;          // [slices][NC * W][tiles * FUSED_TPB]
     double *out;
+    // GEN instantiation: the angles are the L-shaped rest of a two-part plan (the separable kernel took
+    // [0, l_x0) x [0, l_y0) of the n_thx x n_thy plane) and the cube has its own strides
+    int l_x0, l_y0, out_nx;
+    int64_t out_plane;
 };
+
+// (i_x, i_y) of the a-th angle of a fused launch
+template <bool GEN>
+__device__ __forceinline__ void fused_angle_of(const FusedParams &P, int a, int &ix, int &iy) {
+    if (!GEN) { ix = a % P.n_thx; iy = a / P.n_thx; return; }
+    const int rx = P.n_thx - P.l_x0, n1 = rx * P.n_thy;
+    if (a < n1) { ix = P.l_x0 + a % rx; iy = a / rx; }
+    else { const int j = a - n1; ix = j % P.l_x0; iy = P.l_y0 + j / P.l_x0; }
+}
 
 constexpr int FUSED_CHUNK_DBL = HDR + FUSED_SUB * REC;
 constexpr int FUSED_SMEM = FUSED_CHUNK_DBL * 8 + W * FUSED_TPB * 16;      // records + up to 64 omega groups' omega*/2pi
 
-template <int NC, int DEG>
+template <int NC, int DEG, bool GEN>
 __global__ void __launch_bounds__(FUSED_TPB, 4)
 rad_fused_kernel(const FusedParams P) {
     static_assert(FUSED_SUB == FUSED_TPB, "one sample per thread and packing round");
@@ -50,14 +63,16 @@ rad_fused_kernel(const FusedParams P) {
     const int64_t n = b.n;
 
     // ---- this thread's grid coordinates (as in rad_main_kernel: flattened (omega group, angle), angle fastest)
-    const int A = P.n_thx * P.n_thy;
+    const int A = GEN ? angle_count(P.n_thx, P.n_thy, P.l_x0, P.l_y0) : P.n_thx * P.n_thy;
     const int n_wg = (P.n_omega + W - 1) / W;
     const int64_t T = (int64_t)n_wg * A;
     const int64_t t_pad = (int64_t)P.tiles * FUSED_TPB;
     const int64_t gid = (int64_t)blockIdx.x * FUSED_TPB + tid;
     const int64_t gc = min(gid, T - 1);
     const int wg = (int)(gc / A), a = (int)(gc % A);
-    const double nx = P.thx[a % P.n_thx], ny = P.thy[a / P.n_thx];
+    int ix0, iy0;
+    fused_angle_of<GEN>(P, a, ix0, iy0);
+    const double nx = P.thx[ix0], ny = P.thy[iy0];
     const dd h = half_theta2_dd(nx, ny);
     // omega* / 2 pi (double-double: two FP64 divisions each) once per omega the CTA touches, not once per thread:
     // the prologue is paid by every time slice, i.e. dozens of times per tile
@@ -181,9 +196,10 @@ rad_fused_kernel(const FusedParams P) {
         const int wg2 = (int)(g / A), a2 = (int)(g % A);
         const int iw = wg2 * W + j;
         if (live && c == 0 && g < T && iw < P.n_omega) {
-            const double v = spectrum_value<NC>(s, P.thx[a2 % P.n_thx], P.thy[a2 / P.n_thx], P.model,
-                                                P.omega[iw] * P.lam, gamma0);
-            double *dstp = P.out + (int64_t)iw * A + a2;
+            int ix, iy;
+            fused_angle_of<GEN>(P, a2, ix, iy);
+            const double v = spectrum_value<NC>(s, P.thx[ix], P.thy[iy], P.model, P.omega[iw] * P.lam, gamma0);
+            double *dstp = GEN ? P.out + iw * P.out_plane + (int64_t)iy * P.out_nx + ix : P.out + (int64_t)iw * A + a2;
             *dstp = P.accumulate ? *dstp + v : v;
         }
     }

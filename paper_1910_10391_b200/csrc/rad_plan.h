@@ -47,6 +47,8 @@ struct Part {
                               // share the T table through distributed shared memory (needs an even y tile count);
                               // 3 = pairs on neighbouring omega tiles that share the F table (4 accumulators per
                               // point, even omega tile count, cube output); 1 = single CTAs
+    int f_tiles, f_slices;    // > 0: this (direct) part runs through the fused single-launch kernel instead of
+                              // main + ordered reduction: the L-shaped rest of a two-part plan of one short trajectory
 };
 
 struct CallPlan {
@@ -59,7 +61,7 @@ struct CallPlan {
     int launches() const {
         if (fused) return 1;
         int l = 1;            // pack
-        for (int i = 0; i < nparts; ++i) l += 1 + (part[i].plan.mode != MODE_DIRECT);
+        for (int i = 0; i < nparts; ++i) l += part[i].f_tiles > 0 ? 1 : 1 + (part[i].plan.mode != MODE_DIRECT);
         return l;
     }
 };
@@ -127,7 +129,7 @@ static inline void choose_parts(int n_omega, int n_thx, int n_thy, int nc, int k
                                 Part *part, int &nparts) {
     const int ty = nc == 6 ? 8 : 16;
     auto whole = [&](int k) {
-        part[0] = Part{k, n_thx, n_thy, -1, -1, n_thx * n_thy, Plan{}, 0, 1};
+        part[0] = Part{k, n_thx, n_thy, -1, -1, n_thx * n_thy, Plan{}, 0, 1, 0, 0};
         nparts = 1;
     };
     if (kernel == 1) return whole(K_DIRECT);
@@ -153,8 +155,8 @@ static inline void choose_parts(int n_omega, int n_thx, int n_thy, int nc, int k
             }
     }
     if (bx > 0) {
-        part[0] = Part{K_SEP, bx, by, -1, -1, bx * by, Plan{}, 0, 1};
-        part[1] = Part{K_DIRECT, n_thx, n_thy, bx, by, n_thx * n_thy - bx * by, Plan{}, 0, 1};
+        part[0] = Part{K_SEP, bx, by, -1, -1, bx * by, Plan{}, 0, 1, 0, 0};
+        part[1] = Part{K_DIRECT, n_thx, n_thy, bx, by, n_thx * n_thy - bx * by, Plan{}, 0, 1, 0, 0};
         nparts = 2;
         return;
     }
@@ -208,6 +210,20 @@ static inline CallPlan plan_call(int count, int64_t n_max, int n_omega, int n_th
         Part &pt = cp.part[i];
         pt.plan = pt.kernel == K_DIRECT ? split_plan(K_DIRECT, count, cp.cpt, n_omega, pt.angles, 0, nc, sms)
                                         : split_plan(K_SEP, count, cp.cpt, n_omega, pt.n_thx, pt.n_thy, nc, sms);
+        pt.f_tiles = pt.f_slices = 0;
+        if (pt.kernel == K_DIRECT && pt.l_x0 >= 0 && count == 1 && n_max <= 32768) {
+            // the rest of a two-part plan is a small problem of its own: (n_omega / 8) x angles threads.  The fused
+            // kernel evaluates it in one launch with sample-granular time slices (the direct kernel's slices are
+            // whole 128-sample chunks: 24 chunks over 480 CTAs on the paper's grid) and no second pass
+            const int64_t T = (int64_t)((n_omega + PLAN_W - 1) / PLAN_W) * pt.angles;
+            const int64_t t64 = (T + FUSED_TPB - 1) / FUSED_TPB;
+            if (fused_resident > 0 && t64 <= fused_resident) {
+                pt.f_tiles = (int)t64;
+                pt.f_slices = (int)std::max<int64_t>(1, std::min<int64_t>(fused_resident / t64, std::max<int64_t>(1, n_max / 32)));
+                pt.plan.mode = MODE_TSPLIT; pt.plan.p_slices = 1; pt.plan.t_slices = pt.f_slices; pt.plan.tiles = pt.f_tiles;
+                pt.plan.partial_bytes = align_up((size_t)pt.f_slices * nc * PLAN_W * pt.f_tiles * FUSED_TPB * 8, 256);
+            }
+        }
         pt.off_partial = off;
         off += pt.plan.partial_bytes;
         pt.cl = 1;

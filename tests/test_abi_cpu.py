@@ -179,7 +179,7 @@ def test_the_papers_typical_grid_is_split_in_two_parts(radlib):
     d = radlib.rad_plan_describe
     p = d(1, 3000, 100, 50, 50, 0)
     assert (p["kernel"], p["parts"], p["interior_x"], p["interior_y"], p["tiles"], p["slices"]) == (2, 2, 48, 48, 63, 7)
-    assert p["launches"] == 5                         # pack, separable main + reduction, direct main + reduction
+    assert p["launches"] == 4                         # pack, separable main + reduction, fused single launch on the rest
     p = d(1, 3000, 100, 50, 50, 2)                   # spin-1/2: 16 x 16 x 8 tiles, 48 = 6 x 8 rows
     assert (p["parts"], p["interior_x"], p["interior_y"]) == (2, 48, 48)
     assert d(1, 14287, 256, 32, 32, 0)["parts"] == 1 and d(1, 3000, 100, 64, 48, 0)["parts"] == 1
