@@ -104,7 +104,16 @@ def parse():
     return ap.parse_args()
 
 
-def make_workload(name: str, cfg4_count: int = 1000, spin: str = "1/2"):
+def job_evals(wl) -> int:
+    """evals of the WHOLE job: a rank of a sharded cfg4 run holds only its own block of the trajectories."""
+    if wl.batch is not None and "global_count" in wl.meta:
+        return wl.n_points * wl.meta["global_count"] * int(wl.n[0])
+    return wl.evals
+
+
+def make_workload(name: str, cfg4_count: int = 1000, spin: str = "1/2", rank: int = 0, world: int = 1):
+    """rank / world: under torchrun a rank generates only ITS block of cfg4's trajectories (seed of trajectory p is
+    4000 + p wherever it is generated), not the whole 8.8 GB ensemble on every rank."""
     import workloads
     model = workloads.SPIN0 if spin == "0" else workloads.SPIN_HALF
     if name in ("cfg1", "cfg2", "paper_typical"):
@@ -112,6 +121,12 @@ def make_workload(name: str, cfg4_count: int = 1000, spin: str = "1/2"):
     if name in ("cfg3", "cfg5"):
         return workloads.make(name, model=model)
     if name == "cfg4":
+        if world > 1:
+            from paper_1910_10391_b200.sharding import shard_range
+            lo, hi = shard_range(cfg4_count, rank, world)
+            wl = workloads.make("cfg4", count=max(hi - lo, 1), seed0=4000 + lo)
+            wl.meta.update(global_count=cfg4_count, block=(lo, hi))
+            return wl
         return workloads.make("cfg4", count=cfg4_count)
     raise SystemExit(f"unknown workload {name}")
 
@@ -285,6 +300,8 @@ class Bench:
             n_w = hi - lo
         if wl.batch is not None:
             p_lo, p_hi = shard_range(len(wl.n), self.rank, self.world) if shard == "ensemble" else (0, len(wl.n))
+            if "block" in wl.meta:                                     # already this rank's block (make_workload)
+                p_lo, p_hi = 0, wl.meta["block"][1] - wl.meta["block"][0]
             dtr = {k: self.to_dev(v[p_lo:p_hi]) for k, v in wl.batch.items()}
             n_vec = np.ascontiguousarray(wl.n[p_lo:p_hi])
             count, n_max = len(n_vec), int(np.max(n_vec)) if len(n_vec) else 2
@@ -420,8 +437,8 @@ class Bench:
     def entry(self, r, with_direct=None):
         """per_config record of a run (value = whole-job evals/s)."""
         wl = r["wl"]
-        e = {"workload": wl.name, "model": MODELS[wl.model], "evals_per_step": wl.evals,
-             "value": wl.evals * r["steps"] / (r["total_ms"] * 1e-3), "unit": UNIT,
+        e = {"workload": wl.name, "model": MODELS[wl.model], "evals_per_step": job_evals(wl),
+             "value": job_evals(wl) * r["steps"] / (r["total_ms"] * 1e-3), "unit": UNIT,
              "ms_per_step": r["total_ms"] / r["steps"], "steps": r["steps"], "warmup": r["warmup"],
              "launches_per_step": r["launches"] / r["steps"], "plan": r["plan"], "roofline": self.roofline(r),
              "clocks": r["clocks"]}
@@ -517,14 +534,14 @@ def run_b200(args):
     B = Bench(args)
     world, rank = B.world, B.rank
     kopt = {"auto": 0, "direct": 1, "separable": 2, "fused": 3}[args.kernel]
-    wl = make_workload(args.workload, args.cfg4_count, args.spin)
+    wl = make_workload(args.workload, args.cfg4_count, args.spin, rank, world)
     shard = None
     if world > 1:
         shard = "ensemble" if wl.batch is not None else "omega"
     warmup = max(args.warmup, 3)
     head = B.run(wl, args.steps, warmup, kopt, shard)
     step_ms = head["total_ms"] / args.steps
-    value = wl.evals * args.steps / (head["total_ms"] * 1e-3)
+    value = job_evals(wl) * args.steps / (head["total_ms"] * 1e-3)
 
     # the same workload through the direct (one phasor per eval) kernel, for the record: the north_star target
     # (>= 60 % of FP64 peak) is stated for that kernel
@@ -549,7 +566,7 @@ def run_b200(args):
         todo = [("cfg2", "1/2", 20, 3, True), ("cfg3", "1/2", 5, 3, True), ("cfg4", "1/2", 2, 1, False),
                 ("cfg5", "0", 2, 1, False), ("cfg1", "1/2", 50, 5, True), ("paper_typical", "1/2", 20, 3, True)]
         for name, spin, k, w, with_direct in todo:
-            w2 = make_workload(name, args.cfg4_count, spin)
+            w2 = make_workload(name, args.cfg4_count, spin, rank, world)
             sh = None
             if world > 1:
                 sh = "ensemble" if w2.batch is not None else "omega"
@@ -563,7 +580,7 @@ def run_b200(args):
 
     if rank == 0:
         n_max = int(np.max(wl.n)) if wl.batch is not None else len(wl.traj["t"])
-        count = len(wl.n) if wl.batch is not None else 1
+        count = wl.meta.get("global_count", len(wl.n)) if wl.batch is not None else 1
         roof = B.roofline(head)
         if direct is not None and roof is not None:
             roof["direct_kernel_same_run"] = {"kernel": KERNELS[1], "value": wl.evals * direct["steps"] / (direct["total_ms"] * 1e-3),
@@ -578,7 +595,7 @@ def run_b200(args):
             "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
             "data": "synthetic",
             "config": {"workload": wl.name, "model": MODELS[wl.model], "samples": n_max, "trajectories": count,
-                       "grid": [len(wl.omega), len(wl.thy), len(wl.thx)], "evals_per_step": wl.evals,
+                       "grid": [len(wl.omega), len(wl.thy), len(wl.thx)], "evals_per_step": job_evals(wl),
                        "l2": "flushed between steps (256 MiB memset)", "parallelism": par, "plan": head["plan"]},
             "clocks": head["clocks"],
             "e2e": e2e_info,

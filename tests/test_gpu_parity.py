@@ -778,6 +778,19 @@ def test_papers_typical_grid_in_two_parts(rad, oracle_mod, model):
     assert_parity(cube, ref, label=f"paper typical model {model}")
 
 
+@pytest.mark.parametrize("kernel", [0, 1, 2, 3])
+def test_seventeen_cubed_through_every_kernel(rad, oracle_mod, kernel):
+    """17 x 17 x 17: one more than a tile in every direction (the separable kernel pads to 32 x 32 x 32, fill 0.15; the
+    direct kernel has a ragged last omega group of 1; the library's own choice is the fused kernel), spin-1/2, full grid
+    against the oracle through the library's choice and through each kernel forced."""
+    wl = workloads.make("cfg2", n=3000, n_omega=17, n_th=17, seed=21)
+    lam = 0.45 / wl.omega.max()
+    if kernel == 0:
+        assert rad.rad_plan_kernel(17, 17, 17, SH, n_max=3000) == 3
+    cube = run_single(rad, wl, SH, lam, kernel=kernel)
+    assert_parity(cube, oracle_mod.grid(wl.traj, wl.omega, wl.thx, wl.thy, SH, lam), label=f"17^3 kernel {kernel}")
+
+
 def test_two_parts_rectangular_rest_on_one_axis_and_ensemble(rad, oracle_mod):
     """Only one axis leaves a rest (50 x 32: columns 48, 49), n_thx != n_thy, an ensemble with accumulate; against the
     oracle on a sample of points that covers interior, rest and the corners."""

@@ -122,3 +122,22 @@ def test_shard_range_properties():
             assert max(sizes) - min(sizes) <= 1 and sum(sizes) == total
     with pytest.raises(ValueError):
         shard_range(4, 2, 2)
+
+
+def test_bench_generates_each_ranks_block_of_the_ensemble():
+    """bench.py under torchrun: a rank generates only its own block of cfg4's trajectories (seed of trajectory p =
+    4000 + p wherever it is generated); the blocks tile the global ensemble and the job's eval count stays the whole
+    job's.  (Small n: the full-size ensemble is 8.8 GB.)"""
+    import bench
+    import workloads
+    from paper_1910_10391_b200.sharding import shard_range
+    whole = workloads.make("cfg4", count=7, n=50, n_omega=3, n_th=2)
+    for world in (2, 3):
+        for rank in range(world):
+            lo, hi = shard_range(7, rank, world)
+            blk = workloads.make("cfg4", count=hi - lo, n=50, n_omega=3, n_th=2, seed0=4000 + lo)
+            for k in whole.batch:
+                assert np.array_equal(blk.batch[k], whole.batch[k][lo:hi])
+    wl = workloads.make("cfg4", count=2, n=50, n_omega=3, n_th=2, seed0=4003)
+    wl.meta.update(global_count=7, block=(3, 5))
+    assert bench.job_evals(wl) == whole.evals and bench.job_evals(whole) == whole.evals
