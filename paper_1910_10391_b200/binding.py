@@ -394,7 +394,7 @@ def rad_sum_cubes(cubes, accumulate: bool = False, out=None, stream=None):
 def rad_angular_spectrum(batch: dict, n, omega, thx, thy, d_solid_angle: float, theta_cut: float = 0.0,
                          model: int = CLASSICAL, hbarc_over_E=None, out=None, workspace=None, stream=None,
                          kernel: int = 0, profile=None):
-    """dI/dw of an ensemble, slab by slab, without the whole cube in memory."""
+    """dI/dw of an ensemble, formed in the main kernel's epilogue without a cube where the grid fills the GPU."""
     ts = [_dev(batch[k], k) for k in FIELDS]
     count, stride = ts[0].shape
     if any(tuple(t.shape) != (count, stride) for t in ts):

@@ -745,8 +745,11 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const int64
     }
     const int nc = model == RAD_SPIN_HALF ? 6 : 4;
     const CallPlan cp = plan_for(b->count, n_max, g->n_omega, g->n_thx, g->n_thy, nc, kopt, ang != nullptr);
-    if (kopt == RAD_KERNEL_FUSED && (!cp.fused || off_host)) return RAD_EINVAL;
-    const bool fused = cp.fused && !off_host;
+    if (kopt == RAD_KERNEL_FUSED && !cp.fused) return RAD_EINVAL;
+    // (a single section of a sectioned trajectory is one trajectory that starts at off_host[0]: the fused kernel
+    // takes it like any other.  The plan of a fused call overlays the partial amplitudes on the packed buffer it does
+    // not need, so a fused plan must never fall through to the multi-launch path below.)
+    const bool fused = cp.fused;
     if (ang && !(cp.nparts == 1 && cp.part[0].plan.mode == MODE_DIRECT)) return RAD_EINVAL;
     if (workspace && (reinterpret_cast<uintptr_t>(workspace) & 255)) return RAD_EINVAL;
     if (workspace && workspace_bytes < cp.total) return RAD_ENOSPACE;
@@ -762,7 +765,9 @@ static int run_batch(const rad_traj_batch *b, const int64_t *n_host, const int64
 
     if (fused) {              // ---- one cooperative launch does rows a0-a6 (rad_fused.cuh)
         FusedParams fp{};
-        fp.tr = rad_traj{n_host[0], b->t, b->dz, b->x, b->y, b->vx, b->vy, b->dvz, b->ax, b->ay, b->az, b->gamma};
+        const int64_t o = off_host ? off_host[0] : 0;
+        fp.tr = rad_traj{n_host[0], b->t + o, b->dz + o, b->x + o, b->y + o, b->vx + o, b->vy + o, b->dvz + o,
+                         b->ax + o, b->ay + o, b->az + o, b->gamma + o};
         fp.lam = model == RAD_CLASSICAL ? 0.0 : lam_host[0];
         fp.omega = g->omega; fp.thx = g->thx; fp.thy = g->thy;
         fp.n_omega = g->n_omega; fp.n_thx = g->n_thx; fp.n_thy = g->n_thy;

@@ -589,6 +589,16 @@ def test_sections_sum(rad, oracle_mod, kernel):
     both = rad.rad_sections_sum(dev_dict(trs), start[2:], *dev_grid(wl), model=SH, hbarc_over_E=lam[2:],
                                 accumulate=True, out=half, kernel=kernel).cpu().numpy()
     assert_parity(both, ref, label=f"sections accumulate kernel {kernel}")
+    # ONE section that starts inside the trajectory: a single short trajectory at an offset -- the shape the fused
+    # single-launch kernel takes (regression: its plan overlays the partial amplitudes on the unused packed buffer, so
+    # falling through to the multi-launch path with that plan corrupted the records)
+    one = np.array([701, 1500], dtype=np.int64)
+    b1 = {k: tr[k][None, 701:1501].copy() for k in tr}
+    for model in (CL, S0, SH):
+        ref1 = oracle_mod.ensemble_points(b1, np.array([800]), w, nx, ny, model, lam[2:3] if model else None)
+        c1 = rad.rad_sections_sum(dev_dict(trs), one, *dev_grid(wl), model=model, hbarc_over_E=lam[2:3] if model else None,
+                                  kernel=kernel).cpu().numpy()
+        assert_parity(c1, ref1, label=f"one section kernel {kernel} model {model}")
     with pytest.raises(rad.RadError):
         rad.rad_sections_sum(dev_dict(trs), [0, 10, 10], *dev_grid(wl))
     with pytest.raises(rad.RadError):
