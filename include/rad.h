@@ -144,6 +144,11 @@ int rad_semiclassical(const rad_traj *traj, const rad_grid *grid, int spin,
 
 /* out[m] (+)= sum over p (ascending) of the spectrum of trajectory p.
  * hbarc_over_E: HOST array, one per trajectory (NULL allowed iff model is classical).
+ * batch->n and hbarc_over_E are read on the host (they size the launch) and, for count > 1, copied to the device
+ * through `cuda_stream` (cudaMemcpyAsync from the caller's memory): pageable memory is staged by the runtime before
+ * the call returns -- which may make the call wait for earlier work of the stream -- and pinned memory must stay
+ * valid and unchanged until the stream has passed the copy.  Up to 2^31 - 1 trajectories (more than 65 535 are
+ * packed in several passes of one launch).
  * accumulate: 0 overwrites out, 1 adds to it (resume a partial ensemble). */
 int rad_ensemble_sum(const rad_traj_batch *batch, const rad_grid *grid, rad_model model,
                      const double *hbarc_over_E, int accumulate, double *out,
