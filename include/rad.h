@@ -269,8 +269,8 @@ size_t rad_workspace_bytes(int32_t count, int64_t n_max,
  * back once).  Every pointer inside traj/batch/grid and `out` is HOST memory
  * (pinned memory makes the copies asynchronous).  Device buffers come from the
  * stream-ordered pool; the call returns after the result is in `out` (it synchronises the stream once).
- * Arrays that follow one another in host memory in the order of the struct fields (t, dz, x, ..., gamma of one
- * allocation; omega, thx, thy of one allocation) are copied in one transfer instead of eleven / three.
+ * Arrays that follow one another in host memory in the order t, dz, x, y, vx, vy, dvz, ax, ay, az, gamma, omega, thx,
+ * thy (any run of them in one allocation) are copied in one transfer instead of one each.
  * model: rad_model; hbarc_over_E ignored for RAD_CLASSICAL. */
 int rad_eval_host(const rad_traj *traj, const rad_grid *grid, rad_model model,
                   double hbarc_over_E, double *out, const rad_options *opt, void *cuda_stream);

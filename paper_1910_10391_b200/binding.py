@@ -432,33 +432,57 @@ def _host(a, name: str) -> np.ndarray:
     return a
 
 
+def _host_ptr(a, name: str):
+    """(address, shape, keep-alive object) of a contiguous float64 host array or CPU tensor.  The host-buffer calls
+    marshal fifteen arrays per call and a small problem is ~50 us of GPU work: torch's data_ptr() and numpy's
+    __array_interface__ cost a fraction of a microsecond each, `tensor.numpy().ctypes.data` several."""
+    if isinstance(a, torch.Tensor):
+        if a.is_cuda or a.dtype != torch.float64 or not a.is_contiguous():
+            raise TypeError(f"{name}: expected a contiguous float64 CPU tensor")
+        return a.data_ptr(), tuple(a.shape), a
+    a = np.asarray(a)
+    if a.dtype != np.float64 or not a.flags.c_contiguous:
+        raise TypeError(f"{name}: expected a C-contiguous float64 array")
+    return a.__array_interface__["data"][0], a.shape, a
+
+
+def _host_grid_and_out(omega, thx, thy, out, need_out: bool):
+    (pw, sw, kw), (px, sx, kx), (py, sy, ky) = _host_ptr(omega, "omega"), _host_ptr(thx, "thx"), _host_ptr(thy, "thy")
+    if len(sw) != 1 or len(sx) != 1 or len(sy) != 1:
+        raise ValueError("omega, thx, thy must be 1-D")
+    g = _Grid(sw[0], sx[0], sy[0], pw, px, py)
+    if out is None:
+        if need_out:
+            raise ValueError("accumulate needs an existing out")
+        out = np.empty((sw[0], sy[0], sx[0]), dtype=np.float64)
+    po, so, ko = _host_ptr(out, "out")
+    if int(np.prod(so)) != sw[0] * sx[0] * sy[0]:
+        raise ValueError("out has the wrong number of elements")
+    return g, out, po, (kw, kx, ky, ko)
+
+
 def rad_eval_host(traj: dict, omega, thx, thy, model: int = CLASSICAL, hbarc_over_E: float = 0.0,
                   out=None, stream=None, kernel: int = 0, profile=None):
     """Host-buffer call: H2D, evaluate, D2H inside the C library."""
-    hs = [_host(traj[k], k) for k in FIELDS]
-    n = hs[0].shape[0]
-    if any(h.ndim != 1 or h.shape[0] != n for h in hs):
+    hs = [_host_ptr(traj[k], k) for k in FIELDS]
+    shape = hs[0][1]
+    if len(shape) != 1 or any(h[1] != shape for h in hs):
         raise ValueError("trajectory arrays must be 1-D and of one length")
-    w, x, y = _host(omega, "omega"), _host(thx, "thx"), _host(thy, "thy")
-    t = _Traj(n, *[h.ctypes.data for h in hs])
-    g = _Grid(w.size, x.size, y.size, w.ctypes.data, x.ctypes.data, y.ctypes.data)
-    if out is None:
-        out = np.empty((w.size, y.size, x.size), dtype=np.float64)
-    o = _host(out, "out")
-    if o.size != w.size * x.size * y.size:
-        raise ValueError("out has the wrong number of elements")
+    t = _Traj(shape[0], *[h[0] for h in hs])
+    g, out, po, keep = _host_grid_and_out(omega, thx, thy, out, False)
     _check(load_library().rad_eval_host(ctypes.byref(t), ctypes.byref(g), int(model), float(hbarc_over_E),
-                                        o.ctypes.data, _opt(kernel, profile), _stream_ptr(stream)))
+                                        po, _opt(kernel, profile), _stream_ptr(stream)))
     return out
 
 
 def rad_ensemble_sum_host(batch: dict, n, omega, thx, thy, model: int = CLASSICAL, hbarc_over_E=None,
                           accumulate: bool = False, out=None, stream=None, kernel: int = 0, profile=None):
-    hs = [_host(batch[k], k) for k in FIELDS]
-    if hs[0].ndim != 2:
+    hs = [_host_ptr(batch[k], k) for k in FIELDS]
+    shape = hs[0][1]
+    if len(shape) != 2:
         raise ValueError("batch arrays must be 2-D (count, stride)")
-    count, stride = hs[0].shape
-    if any(h.shape != (count, stride) for h in hs):
+    count, stride = shape
+    if any(h[1] != shape for h in hs):
         raise ValueError("batch arrays must share one (count, stride) shape")
     n_host = np.ascontiguousarray(n, dtype=np.int64)
     if n_host.shape != (count,):
@@ -466,19 +490,11 @@ def rad_ensemble_sum_host(batch: dict, n, omega, thx, thy, model: int = CLASSICA
     lam = None
     if hbarc_over_E is not None:
         lam = np.ascontiguousarray(np.broadcast_to(np.asarray(hbarc_over_E, dtype=np.float64), (count,)))
-    w, x, y = _host(omega, "omega"), _host(thx, "thx"), _host(thy, "thy")
-    b = _Batch(count, stride, n_host.ctypes.data, *[h.ctypes.data for h in hs])
-    g = _Grid(w.size, x.size, y.size, w.ctypes.data, x.ctypes.data, y.ctypes.data)
-    if out is None:
-        if accumulate:
-            raise ValueError("accumulate needs an existing out")
-        out = np.empty((w.size, y.size, x.size), dtype=np.float64)
-    o = _host(out, "out")
-    if o.size != w.size * x.size * y.size:
-        raise ValueError("out has the wrong number of elements")
+    b = _Batch(count, stride, n_host.ctypes.data, *[h[0] for h in hs])
+    g, out, po, keep = _host_grid_and_out(omega, thx, thy, out, bool(accumulate))
     _check(load_library().rad_ensemble_sum_host(ctypes.byref(b), ctypes.byref(g), int(model),
                                                 lam.ctypes.data if lam is not None else None,
-                                                1 if accumulate else 0, o.ctypes.data, _opt(kernel, profile),
+                                                1 if accumulate else 0, po, _opt(kernel, profile),
                                                 _stream_ptr(stream)))
     return out
 

@@ -1103,24 +1103,26 @@ int rad_ensemble_sum_host(const rad_traj_batch *b, const rad_grid *g, rad_model 
     CK(pool_alloc(reinterpret_cast<void **>(&dev), (11 * tot + ng + M) * sizeof(double), st));
     PoolScratch pool;
     pool.p = dev; pool.st = st;
+    // Arrays that follow one another in host memory (a caller that keeps its SoA block -- and the grid behind it -- in
+    // one allocation) go over in ONE copy: the device layout is the same sequence t, dz, ..., gamma, omega, thx, thy,
+    // and for a small problem every separate copy costs more than its bytes (config 1: 14 copies ~ 85 us against a
+    // 47 us kernel).
     const double *d[11];
-    // Arrays that follow one another in host memory (a caller that keeps its SoA block in one allocation) go over in
-    // ONE copy: for a small problem the eleven + three separate copies cost more than the kernel (config 1: 14 copies
-    // ~ 85 us against a 47 us kernel).
-    for (int i = 0; i < 11;) {
-        int j = i;
-        while (j + 1 < 11 && src[j + 1] == src[j] + tot) ++j;
-        CK(cudaMemcpyAsync(dev + i * tot, src[i], (size_t)(j - i + 1) * tot * sizeof(double), cudaMemcpyHostToDevice, st));
-        for (int k = i; k <= j; ++k) d[k] = dev + k * tot;
-        i = j + 1;
-    }
     double *gw = dev + 11 * tot, *gx = gw + g->n_omega, *gy = gx + g->n_thx, *dout = gy + g->n_thy;
-    if (g->thx == g->omega + g->n_omega && g->thy == g->thx + g->n_thx) {
-        CK(cudaMemcpyAsync(gw, g->omega, ng * sizeof(double), cudaMemcpyHostToDevice, st));
-    } else {
-        CK(cudaMemcpyAsync(gw, g->omega, g->n_omega * sizeof(double), cudaMemcpyHostToDevice, st));
-        CK(cudaMemcpyAsync(gx, g->thx, g->n_thx * sizeof(double), cudaMemcpyHostToDevice, st));
-        CK(cudaMemcpyAsync(gy, g->thy, g->n_thy * sizeof(double), cudaMemcpyHostToDevice, st));
+    {
+        const double *hsrc[14];
+        size_t cnt[14], off[14];
+        for (int i = 0; i < 11; ++i) { hsrc[i] = src[i]; cnt[i] = tot; off[i] = i * tot; d[i] = dev + i * tot; }
+        hsrc[11] = g->omega; cnt[11] = g->n_omega; off[11] = 11 * tot;
+        hsrc[12] = g->thx;   cnt[12] = g->n_thx;   off[12] = off[11] + g->n_omega;
+        hsrc[13] = g->thy;   cnt[13] = g->n_thy;   off[13] = off[12] + g->n_thx;
+        for (int i = 0; i < 14;) {
+            int j = i;
+            size_t run = cnt[i];
+            while (j + 1 < 14 && hsrc[j + 1] == hsrc[j] + cnt[j]) { ++j; run += cnt[j]; }
+            CK(cudaMemcpyAsync(dev + off[i], hsrc[i], run * sizeof(double), cudaMemcpyHostToDevice, st));
+            i = j + 1;
+        }
     }
     if (accumulate) CK(cudaMemcpyAsync(dout, out, M * sizeof(double), cudaMemcpyHostToDevice, st));
     rad_traj_batch db{b->count, b->stride, b->n, d[0], d[1], d[2], d[3], d[4], d[5], d[6], d[7], d[8], d[9], d[10]};

@@ -254,6 +254,17 @@ def test_host_entry_points(rad, oracle_mod):
     nw, nx_ = len(we.omega), len(we.thx)
     again = rad.rad_ensemble_sum_host(mixed, we.n, gb[:nw], gb[nw:nw + nx_], gb[nw + nx_:])
     assert np.array_equal(again, cube)
+    # everything -- eleven fields and the grid behind them -- in ONE allocation: one transfer
+    per = we.batch["t"].size
+    flat = np.empty(11 * per + gb.size)
+    whole = {}
+    for i, k in enumerate(rad.FIELDS):
+        whole[k] = flat[i * per:(i + 1) * per].reshape(we.batch[k].shape)
+        whole[k][...] = we.batch[k]
+    flat[11 * per:] = gb
+    gf = flat[11 * per:]
+    once = rad.rad_ensemble_sum_host(whole, we.n, gf[:nw], gf[nw:nw + nx_], gf[nw + nx_:])
+    assert np.array_equal(once, cube)
 
 
 # ------------------------------------------------------------------ angular sum (NEXT-1)
