@@ -245,7 +245,12 @@ def run_reference(args):
     line = {"metric": METRIC, "value": value, "unit": UNIT, "impl": "reference", "n_gpus": args.gpus,
             "steps": args.steps, "warmup": args.warmup, "ms_per_step": 1e3 * total_t / args.steps,
             "higher_is_better": True, "scaling": "strong", "vs_baseline": None, "dtype": "f64",
-            "data": "synthetic", "config": {"workload": wl.name, "sample_points_per_step": got},
+            "data": "synthetic",
+            "config": {"workload": wl.name, "model": MODELS[wl.model], "samples": int(np.max(wl.n)) if wl.batch is not None else samples,
+                       "trajectories": len(wl.n) if wl.batch is not None else 1,
+                       "grid": [len(wl.omega), len(wl.thy), len(wl.thx)], "evals_per_step": got * samples,
+                       "sample_points_per_step": got,
+                       "note": "same workload as the b200 arm; each step evaluates a seeded sample of its grid points"},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
             "gpu_launches": 0}
