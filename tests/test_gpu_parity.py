@@ -616,6 +616,62 @@ def test_sections_sum(rad, oracle_mod, kernel):
         rad.rad_sections_sum(dev_dict(trs), [0, 3000], *dev_grid(wl))
 
 
+# ------------------------------------------------------------------ seeded random shapes
+@pytest.mark.parametrize("seed", [11, 12, 13])
+def test_random_shapes_models_kernels_and_entry_points(rad, oracle_mod, seed):
+    """120 seeded random cases per seed: grid shapes around the tile edges (1 ... 51 angles per axis, 1 ... 69 omegas),
+    trajectory lengths around the chunk edges, all three models, the library's kernel choice and each kernel forced,
+    single trajectories, ragged ensembles (with and without accumulate in two calls) and single sections at an offset --
+    the launch plans this reaches include time and trajectory splits, cluster pairs along theta_y and along omega, and
+    the fused kernel.  Sampled points (always the arg-max and both corners) against the oracle.  (A longer unseeded
+    run of the same generator found the single-section bug fixed in rad.cu's run_batch.)"""
+    import torch
+    rng = np.random.Generator(np.random.PCG64(seed))
+    for case in range(120):
+        model = int(rng.integers(0, 3)); kernel = int(rng.choice([0, 0, 0, 1, 2]))
+        n = int(rng.choice([2, 3, 127, 128, 129, 500, 1025, 2600]))
+        nw, nx, ny = int(rng.integers(1, 70)), int(rng.integers(1, 52)), int(rng.integers(1, 52))
+        kind = str(rng.choice(["single", "single", "ensemble", "section"]))
+        cnt = int(rng.integers(1, 6)) if kind == "ensemble" else 1
+        we = workloads.make("cfg4", count=cnt, n=n, n_omega=nw, n_th=max(nx, ny), seed0=int(rng.integers(1, 5000)))
+        thx, thy = we.thx[:nx].copy(), we.thy[max(nx, ny) - ny:].copy()
+        g = [torch.from_numpy(a).cuda() for a in (we.omega, thx, thy)]
+        lam = rng.uniform(0.05, 0.8, size=cnt) / we.omega.max() if model else None
+        nvec = rng.integers(2, n + 1, size=cnt).astype(np.int64) if kind == "ensemble" else np.array([n], dtype=np.int64)
+        batch = we.batch
+        if kind == "single":
+            tr = {k: v[0] for k, v in batch.items()}
+            cube = run_single(rad, types_workload(tr, we.omega, thx, thy), model, None if lam is None else float(lam[0]), kernel)
+        elif kind == "section":
+            lo = int(rng.integers(0, n - 1)); hi = int(rng.integers(lo + 1, n))
+            tr = {k: v[0] for k, v in batch.items()}
+            cube = rad.rad_sections_sum(dev_dict(tr), [lo, hi], *g, model=model, hbarc_over_E=lam, kernel=kernel).cpu().numpy()
+            batch = {k: v[:, lo:hi + 1].copy() for k, v in batch.items()}
+            nvec = np.array([hi - lo + 1], dtype=np.int64)
+        else:
+            b = dev_dict(batch)
+            cut = int(rng.integers(0, cnt + 1))
+            if 0 < cut < cnt:
+                first = rad.rad_ensemble_sum({k: v[:cut].contiguous() for k, v in b.items()}, nvec[:cut], *g, model=model,
+                                             hbarc_over_E=None if lam is None else lam[:cut], kernel=kernel)
+                cube = rad.rad_ensemble_sum({k: v[cut:].contiguous() for k, v in b.items()}, nvec[cut:], *g, model=model,
+                                            hbarc_over_E=None if lam is None else lam[cut:], accumulate=True, out=first,
+                                            kernel=kernel).cpu().numpy()
+            else:
+                cube = rad.rad_ensemble_sum(b, nvec, *g, model=model, hbarc_over_E=lam, kernel=kernel).cpu().numpy()
+        flat = cube.ravel()
+        idx = np.unique(np.concatenate([rng.integers(0, flat.size, size=min(flat.size, 20)), [int(np.argmax(flat)), 0, flat.size - 1]]))
+        iw, iy, ix = np.unravel_index(idx, cube.shape)
+        ref = oracle_mod.ensemble_points(batch, nvec, we.omega[iw], thx[ix], thy[iy], model, lam)
+        assert_parity(cube, ref, idx, label=f"random seed {seed} case {case}: {kind} n={n} grid {nw}x{ny}x{nx} model {model} kernel {kernel}")
+
+
+def types_workload(traj, omega, thx, thy):
+    """The few attributes run_single reads, for a trajectory that did not come from workloads.make."""
+    import types
+    return types.SimpleNamespace(traj=traj, omega=omega, thx=thx, thy=thy)
+
+
 # ------------------------------------------------------------------ extreme shapes the paper names
 def test_three_thousand_squared_angles(rad, oracle_mod):
     """"more than 3000^2" angular points without multiple scattering.  2 omegas x 3000 x 3000
