@@ -501,9 +501,9 @@ class Bench:
 def generator_throughput(B):
     """rad_generate_trajectories on its own -- 2000 particles (the paper's ensembles: up to
     2000 particles) x 20 000 steps in each of the three synthetic wells, device time by CUDA events.
-    One thread per particle and a serial recurrence per step: the bound is the latency of that dependent chain, not
-    HBM; the HBM figure (88 B written per particle and step against the measured copy bandwidth) is reported so that
-    this is visible."""
+    One thread per particle and a serial recurrence per step (stores staged through shared memory and written
+    transposed, rad_traj.cuh): the bound is the latency of that dependent chain, not HBM; the HBM figure (88 B written
+    per particle and step against the measured copy bandwidth) is reported so that this is visible."""
     import math
     torch, rad = B.torch, B.rad
     try:

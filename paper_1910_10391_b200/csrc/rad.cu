@@ -1056,13 +1056,13 @@ int rad_generate_trajectories(rad_well well, double kappa, double length, double
         if (!p || !aligned8(p)) return RAD_EINVAL;
     cudaStream_t st = static_cast<cudaStream_t>(cuda_stream);
     const TrajOut o{out->t, out->dz, out->x, out->y, out->vx, out->vy, out->dvz, out->ax, out->ay, out->az, out->gamma};
-    const unsigned blocks = (unsigned)((count + 127) / 128);
+    const unsigned blocks = (unsigned)((count + 31) / 32);            // one warp per CTA (rad_traj.cuh TrajStage)
     if (well == RAD_WELL_HARMONIC_MS)
-        rad_traj_ms_kernel<<<blocks, 128, 0, st>>>(kappa, gamma, dt, sigma, seed, count, n, stride, x0, y0, vx0, vy0, o);
+        rad_traj_ms_kernel<<<blocks, 32, 0, st>>>(kappa, gamma, dt, sigma, seed, count, n, stride, x0, y0, vx0, vy0, o);
     else if (well == RAD_WELL_COSINE)
-        rad_traj_kernel<0><<<blocks, 128, 0, st>>>(kappa, length, gamma, dt, count, n, stride, x0, y0, vx0, vy0, o);
+        rad_traj_kernel<0><<<blocks, 32, 0, st>>>(kappa, length, gamma, dt, count, n, stride, x0, y0, vx0, vy0, o);
     else
-        rad_traj_kernel<1><<<blocks, 128, 0, st>>>(kappa, length, gamma, dt, count, n, stride, x0, y0, vx0, vy0, o);
+        rad_traj_kernel<1><<<blocks, 32, 0, st>>>(kappa, length, gamma, dt, count, n, stride, x0, y0, vx0, vy0, o);
     ++g_launches;
     CK(cudaGetLastError());
     return RAD_OK;
