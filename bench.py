@@ -104,6 +104,21 @@ def parse():
     return ap.parse_args()
 
 
+def inputs_hash(wl) -> str:
+    """blake2b-64 over the arrays this process evaluates (trajectory fields in rad_traj order, n, grid): the arrays, not
+    the recipe, are the inputs of record.  Under torchrun a cfg4 rank hashes its own block."""
+    import hashlib
+    h = hashlib.blake2b(digest_size=8)
+    src = wl.batch if wl.batch is not None else wl.traj
+    for k in ("t", "dz", "x", "y", "vx", "vy", "dvz", "ax", "ay", "az", "gamma"):
+        h.update(np.ascontiguousarray(src[k]).view(np.uint8).reshape(-1).data)
+    if wl.batch is not None:
+        h.update(np.ascontiguousarray(wl.n, dtype=np.int64).view(np.uint8).data)
+    for a in (wl.omega, wl.thx, wl.thy):
+        h.update(np.ascontiguousarray(a).view(np.uint8).data)
+    return h.hexdigest()
+
+
 def job_evals(wl) -> int:
     """evals of the WHOLE job: a rank of a sharded cfg4 run holds only its own block of the trajectories."""
     if wl.batch is not None and "global_count" in wl.meta:
@@ -249,7 +264,7 @@ def run_reference(args):
             "config": {"workload": wl.name, "model": MODELS[wl.model], "samples": int(np.max(wl.n)) if wl.batch is not None else samples,
                        "trajectories": len(wl.n) if wl.batch is not None else 1,
                        "grid": [len(wl.omega), len(wl.thy), len(wl.thx)], "evals_per_step": got * samples,
-                       "sample_points_per_step": got,
+                       "sample_points_per_step": got, "inputs_blake2b64": inputs_hash(wl),
                        "note": "same workload as the b200 arm; each step evaluates a seeded sample of its grid points"},
             "cpu_baseline": {"value": value, "unit": UNIT, "cores": cores, "kind": "oracle", "sample": sample},
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
@@ -442,7 +457,7 @@ class Bench:
     def entry(self, r, with_direct=None):
         """per_config record of a run (value = whole-job evals/s)."""
         wl = r["wl"]
-        e = {"workload": wl.name, "model": MODELS[wl.model], "evals_per_step": job_evals(wl),
+        e = {"workload": wl.name, "model": MODELS[wl.model], "evals_per_step": job_evals(wl), "inputs_blake2b64": inputs_hash(wl),
              "value": job_evals(wl) * r["steps"] / (r["total_ms"] * 1e-3), "unit": UNIT,
              "ms_per_step": r["total_ms"] / r["steps"], "steps": r["steps"], "warmup": r["warmup"],
              "launches_per_step": r["launches"] / r["steps"], "plan": r["plan"], "roofline": self.roofline(r),
@@ -604,6 +619,7 @@ def run_b200(args):
             "data": "synthetic",
             "config": {"workload": wl.name, "model": MODELS[wl.model], "samples": n_max, "trajectories": count,
                        "grid": [len(wl.omega), len(wl.thy), len(wl.thx)], "evals_per_step": job_evals(wl),
+                       "inputs_blake2b64": inputs_hash(wl),
                        "l2": "flushed between steps (256 MiB memset)", "parallelism": par, "plan": head["plan"]},
             "clocks": head["clocks"],
             "e2e": e2e_info,
