@@ -197,7 +197,7 @@ class ClockSampler:
 
 
 # ----------------------------------------------------------------------------- CPU oracle legs
-def oracle_sample_rate(wl, n_points: int, variant: str, repeats: int = 1):
+def oracle_sample_rate(wl, n_points: int, variant: str, repeats: int = 1, keep: dict | None = None):
     """evals/s of the CPU oracle on a seeded subset of the workload's grid points."""
     import oracle
     import workloads
@@ -207,18 +207,22 @@ def oracle_sample_rate(wl, n_points: int, variant: str, repeats: int = 1):
     for _ in range(repeats):
         t0 = time.perf_counter()
         if wl.batch is not None:
-            oracle.ensemble_points(wl.batch, wl.n, w, nx, ny, wl.model,
-                                   wl.hbarc_over_E if wl.model else None, variant=variant)
+            vals = oracle.ensemble_points(wl.batch, wl.n, w, nx, ny, wl.model,
+                                          wl.hbarc_over_E if wl.model else None, variant=variant)
             samples = int(np.sum(wl.n))
         else:
-            oracle.points(wl.traj, w, nx, ny, wl.model, wl.hbarc_over_E, variant=variant)
+            vals = oracle.points(wl.traj, w, nx, ny, wl.model, wl.hbarc_over_E, variant=variant)
             samples = len(wl.traj["t"])
         dt = time.perf_counter() - t0
         best = dt if best is None else min(best, dt)
+    if keep is not None:
+        keep["idx"], keep["values"] = idx, np.asarray(vals, dtype=np.float64)
     return len(idx) * samples / best, len(idx), best
 
 
-def cpu_baseline(wl):
+def cpu_baseline(wl, gpu_cube=None):
+    """gpu_cube: the cube the timed steps wrote (numpy): the long-double oracle values computed here anyway are then
+    also a parity check of THIS run (BASELINE.json tolerance), reported under "parity_in_this_run"."""
     import oracle
     samples = int(np.sum(wl.n)) if wl.batch is not None else len(wl.traj["t"])
     # size the sample for roughly 10-20 s of wall time on this box
@@ -227,8 +231,16 @@ def cpu_baseline(wl):
     oracle_sample_rate(wl, min(npts, 64), "f64")                       # page in / warm up
     rate, got, secs = oracle_sample_rate(wl, npts, "f64")
     npts_ld = max(16, npts // 16)
-    rate_ld, got_ld, secs_ld = oracle_sample_rate(wl, npts_ld, "ld")
-    return {"value": rate, "unit": UNIT, "cores": oracle.threads("f64"), "kind": "oracle",
+    kept = {}
+    rate_ld, got_ld, secs_ld = oracle_sample_rate(wl, npts_ld, "ld", keep=kept)
+    parity = None
+    if gpu_cube is not None:
+        flat = np.asarray(gpu_cube, dtype=np.float64).ravel()
+        got, ref = flat[kept["idx"]], kept["values"].ravel()
+        tol = np.maximum(1e-9 * np.abs(ref), 1e-12 * float(np.max(flat)))
+        parity = {"points": int(len(ref)), "worst_err_over_tol": float(np.max(np.abs(got - ref) / tol)),
+                  "tolerance": "max(1e-9 |oracle|, 1e-12 max(cube)), long-double oracle", "ok": bool(np.all(np.abs(got - ref) <= tol))}
+    return {"value": rate, "unit": UNIT, "cores": oracle.threads("f64"), "kind": "oracle", "parity_in_this_run": parity,
             "sample": (f"{got} seeded grid points x {samples} samples of {wl.name}, double build of "
                        f"oracle/rad_oracle.c (-O2, OpenMP), {secs:.1f} s; long-double build (the parity "
                        f"truth): {rate_ld:.3e} evals/s on {got_ld} points, {secs_ld:.1f} s"),
@@ -379,6 +391,7 @@ class Bench:
             rank_ms = [float(x.item()) / steps for x in all_t]
             total_ms = max(float(x.item()) for x in all_t)
         plan = rad.rad_plan_describe(max(count, 1), n_max, max(n_w, 1), len(wl.thx), len(wl.thy), model, kernel)
+        self.last_cube = out if shard is None else None
         return {"wl": wl, "steps": steps, "warmup": warmup, "total_ms": total_ms, "main_ms": main_ms, "launches": launches,
                 "clocks": clk.summary(), "plan": plan, "rank_ms_per_step": rank_ms, "local_points": n_w * len(wl.thx) * len(wl.thy),
                 "local_samples": int(np.sum(n_vec)) if n_vec is not None else n_max, "shard": shard}
@@ -563,6 +576,7 @@ def run_b200(args):
         shard = "ensemble" if wl.batch is not None else "omega"
     warmup = max(args.warmup, 3)
     head = B.run(wl, args.steps, warmup, kopt, shard)
+    head_cube = B.last_cube.cpu().numpy() if B.last_cube is not None else None
     step_ms = head["total_ms"] / args.steps
     value = job_evals(wl) * args.steps / (head["total_ms"] * 1e-3)
 
@@ -633,7 +647,7 @@ def run_b200(args):
             if world == 1:
                 line["trajectory_generator"] = generator_throughput(B)
         if not args.no_cpu_baseline and world == 1:
-            line["cpu_baseline"] = cpu_baseline(wl)
+            line["cpu_baseline"] = cpu_baseline(wl, head_cube)
         print(json.dumps(line))
     if world > 1:
         B.dist.destroy_process_group()
