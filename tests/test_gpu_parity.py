@@ -616,6 +616,46 @@ def test_sections_sum(rad, oracle_mod, kernel):
         rad.rad_sections_sum(dev_dict(trs), [0, 3000], *dev_grid(wl))
 
 
+def test_concurrent_host_threads_with_different_options(rad):
+    """include/rad.h: no process-wide switch, per-call options, "two threads may call with different options".  Four
+    host threads (ctypes releases the GIL during the call), each on its own stream with its own kernel option, model
+    and grid, 25 calls each; every result equals the serial one bit for bit."""
+    import threading
+    import torch
+    jobs = []
+    for i, (kernel, model, shape) in enumerate([(1, CL, dict(n=900, n_omega=24, n_th=9)), (2, SH, dict(n=1100, n_omega=32, n_th=16)),
+                                                (3, S0, dict(n=1500, n_omega=20, n_th=6)), (0, SH, dict(n=700, n_omega=40, n_th=20))]):
+        wl = workloads.make("cfg2", seed=50 + i, **shape)
+        lam = 0.4 / wl.omega.max()
+        tr, g = dev_dict(wl.traj), dev_grid(wl)
+        call = (lambda tr=tr, g=g, kernel=kernel, model=model, lam=lam, **kw:
+                rad.rad_classical(tr, *g, kernel=kernel, **kw) if model == CL
+                else rad.rad_semiclassical(tr, *g, 0 if model == S0 else 1, lam, kernel=kernel, **kw))
+        jobs.append((call, call().clone()))
+    torch.cuda.synchronize()
+    errors = []
+
+    def worker(call, ref):
+        try:
+            st = torch.cuda.Stream()
+            with torch.cuda.stream(st):
+                for _ in range(25):
+                    out = call(stream=st)
+                    st.synchronize()
+                    if not torch.equal(out, ref):
+                        errors.append("result differs from the serial call")
+                        return
+        except Exception as e:                                   # noqa: BLE001 -- reported below
+            errors.append(repr(e))
+
+    threads = [threading.Thread(target=worker, args=j) for j in jobs]
+    for t in threads:
+        t.start()
+    for t in threads:
+        t.join()
+    assert not errors, errors
+
+
 # ------------------------------------------------------------------ seeded random shapes
 @pytest.mark.parametrize("seed", [11, 12, 13])
 def test_random_shapes_models_kernels_and_entry_points(rad, oracle_mod, seed):
